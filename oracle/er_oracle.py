@@ -1,0 +1,244 @@
+"""CPU ORACLE -- TEST INFRASTRUCTURE ONLY.
+
+A plain, slow, obviously-correct numpy implementation of what the hot path of
+EfficientRollout's self-speculative decoding computes.  It is independent of the
+CUDA path: it shares no code, header, table or helper with
+`paper_2606_18967_b200/csrc`, and nothing under the product package imports it.
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s cpu_baseline /
+`--impl reference` legs may import this module.
+
+What the paper fixes and what it leaves open is listed in DESIGN.md
+("Readings of the paper"); each function cites the passage it follows.
+
+Parity pins (tests/test_oracle_*.py, `-m "not gpu"`):
+  quantize_pack   pinned: error bound |w - q s| <= s/2, idempotent special case,
+                  scale doubling, sign symmetry, brute force over all 2^16 bf16
+                  values against exact rational arithmetic, nibble round trip.
+  w4a16_gemm      pinned: one-hot read-out, exact-integer probe, pure-Python
+                  Fraction brute force on tiny shapes, K-split invariance.
+  spec_verify     pinned: q = p accepts everything, one-hot / zero-probability
+                  cases, exact rational enumeration showing the output
+                  distribution equals p (the theorem of ref. [29] the paper
+                  relies on), scipy softmax.
+  block_efficiency pinned to the values the paper prints (Table 2).
+No function here is "parity unpinned".
+"""
+from __future__ import annotations
+
+import numpy as np
+
+GROUP = 128          # quantization group along K (BASELINE.json north_star; Q2)
+QMAX = 7             # symmetric int4: scale = amax / 7 (BASELINE.json configs[0])
+PACK_PERM = (0, 2, 4, 6, 1, 3, 5, 7)   # nibble i of a word holds logical k = 8 j + PACK_PERM[i] (Q11)
+
+
+# ----------------------------------------------------------------------------
+# bf16 helpers (the oracle's own; bf16 is the upper 16 bits of an IEEE fp32)
+# ----------------------------------------------------------------------------
+
+def bf16_to_f32(u16: np.ndarray) -> np.ndarray:
+    """Exact widening: bf16 bit pattern (uint16) -> float32."""
+    u16 = np.asarray(u16, dtype=np.uint16)
+    return (u16.astype(np.uint32) << np.uint32(16)).view(np.float32)
+
+
+def f32_to_bf16_rne(x: np.ndarray) -> np.ndarray:
+    """float32 -> bf16 bit pattern, round-to-nearest-even on the dropped 16 bits
+    (finite inputs; NaN is outside the contract, Q9)."""
+    b = np.asarray(x, dtype=np.float32).view(np.uint32).astype(np.uint64)
+    lsb = (b >> np.uint64(16)) & np.uint64(1)
+    b = b + np.uint64(0x7FFF) + lsb
+    return (b >> np.uint64(16)).astype(np.uint16)
+
+
+# ----------------------------------------------------------------------------
+# (2) drafter refresh: RTN W4, group 128 along K  ("lightweight RTN
+#     quantization to the FFN and QKVO projection layers", L150 Alg.1 line 3,
+#     L429 "vanilla round-to-nearest (RTN) 4-bit"; layout per DESIGN.md Q1-Q12)
+# ----------------------------------------------------------------------------
+
+def quantize_codes(w_u16: np.ndarray, group: int = GROUP):
+    """bf16 W[N][K] (uint16 bit patterns) -> (codes int8 [N][K] in [-8,7],
+    scales uint16 bf16 bit patterns [K/group][N]).
+
+    Per group of `group` consecutive k of one row (Q2):
+      amax = max |float(w)|                                     (Q3)
+      s    = bf16_RNE( fp32(amax) / fp32(7) )   IEEE fp32 divide (Q4)
+      q    = clamp( rint( fp32(w) / fp32(s) ), -8, 7 )  ties-to-even, divide by
+             the ROUNDED scale, IEEE fp32 divide                 (Q5-Q7)
+      s == 0  ->  all q = 0, s stored +0                         (Q8)
+    """
+    w_u16 = np.asarray(w_u16, dtype=np.uint16)
+    N, K = w_u16.shape
+    assert K % group == 0
+    G = K // group
+    w = bf16_to_f32(w_u16).reshape(N, G, group)
+    amax = np.max(np.abs(w), axis=2)                                   # [N][G] fp32, exact
+    s_u16 = f32_to_bf16_rne(amax / np.float32(QMAX))                   # fp32 IEEE division
+    s = bf16_to_f32(s_u16)                                             # rounded scale, as fp32
+    safe = np.where(s == 0, np.float32(1), s)
+    with np.errstate(invalid="ignore"):
+        ratio = (w / safe[:, :, None]).astype(np.float32)              # fp32 IEEE division
+    q = np.rint(ratio)                                                 # round-half-to-even
+    q = np.clip(q, -8, 7)
+    q = np.where((s == 0)[:, :, None], np.float32(0), q)
+    codes = q.astype(np.int8).reshape(N, K)
+    s_u16 = np.where(s == 0, np.uint16(0), s_u16)
+    return codes, np.ascontiguousarray(s_u16.T)                        # scales [G][N]
+
+
+def pack_codes(codes: np.ndarray) -> np.ndarray:
+    """int8 codes [N][K] in [-8,7] -> uint32 qweight [N][K/8] (ER_PACK_V1, DESIGN.md
+    Q10-Q11): stored nibble u = q + 8 (offset binary); word (n, j) carries logical
+    k = 8 j + PACK_PERM[i] in bits [4 i, 4 i + 4)."""
+    codes = np.asarray(codes, dtype=np.int8)
+    N, K = codes.shape
+    assert K % 8 == 0
+    u = (codes.astype(np.int32) + 8).astype(np.uint32).reshape(N, K // 8, 8)
+    word = np.zeros((N, K // 8), dtype=np.uint32)
+    for i in range(8):
+        word |= u[:, :, PACK_PERM[i]] << np.uint32(4 * i)
+    return word
+
+
+def unpack_codes(qweight: np.ndarray) -> np.ndarray:
+    """Inverse of pack_codes: uint32 [N][K/8] -> int8 [N][K]."""
+    qweight = np.asarray(qweight, dtype=np.uint32)
+    N, J = qweight.shape
+    codes = np.empty((N, J, 8), dtype=np.int8)
+    for i in range(8):
+        nib = (qweight >> np.uint32(4 * i)) & np.uint32(0xF)
+        codes[:, :, PACK_PERM[i]] = nib.astype(np.int32) - 8
+    return codes.reshape(N, J * 8)
+
+
+def quantize_pack(w_u16: np.ndarray, group: int = GROUP):
+    """The refresh call: bf16 W[N][K] -> (qweight uint32 [N][K/8], scales bf16 bits [K/group][N])."""
+    codes, scales = quantize_codes(w_u16, group)
+    return pack_codes(codes), scales
+
+
+# ----------------------------------------------------------------------------
+# (1) drafter linear: y = X . dequant(Wq)^T  (BASELINE.json north_star; PAPER.md:L99-L101,
+#     L175 "Marlin weight-only quantization kernel", L467 "on-the-fly dequantization")
+# ----------------------------------------------------------------------------
+
+def dequantize(qweight: np.ndarray, scales_u16: np.ndarray, group: int = GROUP) -> np.ndarray:
+    """fp64 W_d[N][K] = q[n][k] * float(s[k // group][n]); exact (4-bit x 8-bit significand)."""
+    codes = unpack_codes(qweight).astype(np.float64)
+    s = bf16_to_f32(scales_u16).astype(np.float64)                     # [G][N]
+    return codes * np.repeat(s.T, group, axis=1)
+
+
+def w4a16_gemm(x_u16: np.ndarray, qweight: np.ndarray, scales_u16: np.ndarray, group: int = GROUP) -> np.ndarray:
+    """y_ref[m][n] = sum_k double(x[m][k]) * (double(q[n][k]) * double(s[k//group][n])),
+    fp64 [M][N].  The definition written out; the contraction itself is numpy's fp64 matmul
+    (a library primitive used as one step, no blocking or reordering of ours)."""
+    x = bf16_to_f32(x_u16).astype(np.float64)
+    return x @ dequantize(qweight, scales_u16, group).T
+
+
+# ----------------------------------------------------------------------------
+# (3) speculative verification by rejection sampling  ("preserves the
+#     target-model distribution through rejection sampling"; L445 accept / first
+#     rejection resampled "from the adjusted target distribution" / bonus token;
+#     L544 exact SD needs the full distribution at the rejected position, ref. [29])
+# ----------------------------------------------------------------------------
+
+def softmax64(logits, temperature: float = 1.0) -> np.ndarray:
+    """fp64 softmax over the last axis of float32(logits)/T with max-subtraction (V7)."""
+    z = np.asarray(logits, dtype=np.float32).astype(np.float64) / np.float64(temperature)
+    z = z - np.max(z, axis=-1, keepdims=True)
+    e = np.exp(z)
+    return e / np.sum(e, axis=-1, keepdims=True)
+
+
+def spec_verify(target, draft, draft_tokens, u_accept, u_sample, *, inputs_are_logits: bool,
+                temperature: float = 1.0, return_diag: bool = False):
+    """Textbook speculative rejection sampling, one sequence at a time.
+
+    target [B][gamma+1][V], draft [B][gamma][V]: float32 probabilities, or logits (any
+    float dtype already widened to float32 by the caller) when inputs_are_logits.
+    draft_tokens int32 [B][gamma]; u_accept fp32 [B][gamma] in [0,1); u_sample fp32 [B].
+
+    Steps (V1-V12):
+      1. p_i, q_i in fp64 (softmax64 for logits; widening for probabilities).
+      2. n = 0; for i = 1..gamma: accept iff fp32(u_i) * fp32(q_i(x_i)) < fp32(p_i(x_i))
+         -- one fp32 multiply, then a strict compare; stop at the first failure.
+      3. n < gamma: w = max(0, p_{n+1} - q_{n+1});  n == gamma: w = p_{gamma+1} (bonus).
+         R = sum_v w(v); if R == 0 fall back to w = p_{n+1}.
+      4. token = min{ v : C(v) > r R },  C = inclusive prefix sum of w in vocab order.
+      5. accept_count = n; out_tokens = x_1..x_n, token, then -1 padding.
+    """
+    target = np.asarray(target)
+    draft = np.asarray(draft)
+    B, G1, V = target.shape
+    gamma = G1 - 1
+    assert draft.shape == (B, gamma, V)
+    x = np.asarray(draft_tokens, dtype=np.int64).reshape(B, gamma)
+    ua = np.asarray(u_accept, dtype=np.float32).reshape(B, gamma)
+    us = np.asarray(u_sample, dtype=np.float32).reshape(B)
+
+    accept_count = np.zeros(B, dtype=np.int32)
+    out_tokens = np.full((B, gamma + 1), -1, dtype=np.int32)
+    diag = []
+    for b in range(B):
+        if inputs_are_logits:
+            p = softmax64(target[b], temperature)
+            q = softmax64(draft[b], temperature)
+        else:
+            p = target[b].astype(np.float64)
+            q = draft[b].astype(np.float64)
+        n = 0
+        margins = []
+        for i in range(gamma):
+            pf = np.float32(p[i, x[b, i]])
+            qf = np.float32(q[i, x[b, i]])
+            lhs = np.float32(ua[b, i] * qf)          # fp32 multiply, round to nearest
+            margins.append(abs(float(lhs) - float(pf)) / max(float(pf), 1e-300))
+            if lhs < pf:
+                n += 1
+            else:
+                break
+        if n < gamma:
+            w = np.maximum(0.0, p[n] - q[n])
+        else:
+            w = p[gamma].copy()
+        R = float(np.sum(w))
+        if R == 0.0:
+            w = p[n].copy()
+            R = float(np.sum(w))
+        C = np.cumsum(w)                             # fp64, ascending v
+        thr = float(us[b]) * R
+        tok = int(np.searchsorted(C, thr, side="right"))   # first v with C(v) > thr
+        tok = min(tok, V - 1)
+        accept_count[b] = n
+        out_tokens[b, :n] = x[b, :n]
+        out_tokens[b, n] = tok
+        if return_diag:
+            diag.append({"margins": margins, "C": C, "R": R, "w": w, "r": float(us[b])})
+    if return_diag:
+        return accept_count, out_tokens, diag
+    return accept_count, out_tokens
+
+
+def token_in_widened_interval(d: dict, token: int, slack: float = 1e-5) -> bool:
+    """Rule V10: a device token t' that differs from the oracle's passes iff
+    w(t') > 0 and r lies in t' 's own fp64 CDF interval widened by `slack` on both sides:
+    C(t'-1)/R - slack <= r < C(t')/R + slack."""
+    C, R, w, r = d["C"], d["R"], d["w"], d["r"]
+    if token < 0 or token >= len(C) or not (w[token] > 0):
+        return False
+    lo = (C[token - 1] if token > 0 else 0.0) / R
+    hi = C[token] / R
+    return (lo - slack) <= r < (hi + slack)
+
+
+# ----------------------------------------------------------------------------
+# block efficiency: tau = (1 - alpha^(gamma+1)) / (1 - alpha)
+# ----------------------------------------------------------------------------
+
+def block_efficiency(alpha: float, gamma: float) -> float:
+    if alpha == 1.0:
+        return gamma + 1.0
+    return (1.0 - alpha ** (gamma + 1.0)) / (1.0 - alpha)
