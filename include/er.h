@@ -1,0 +1,135 @@
+/*
+ * er.h -- C ABI of the B200-native hot path of EfficientRollout's self-speculative decoding
+ * (arxiv/paper_2606_18967).  Three operations, named by BASELINE.json's north_star:
+ *
+ *   er_quantize_pack   per-RL-step drafter refresh: bf16 linear weight -> RTN int4 (g128) + bf16 scales
+ *                      PAPER.md:L101 (sec. 4.1 "lightweight RTN quantization to the FFN and QKVO projection
+ *                      layers"), L150 (Alg. 1 line 3), L429 ("vanilla round-to-nearest (RTN) 4-bit")
+ *   er_w4a16_gemm      drafter linear  Y = X . dequant(Wq)^T  at M = 1..256 rows
+ *                      PAPER.md:L99-L101 (dense projections ~90 % of tail decode latency, weight loading
+ *                      dominates), L175 (W4A16 weight-only kernel), L467 (on-the-fly dequantization)
+ *   er_spec_verify     speculative-decoding verification by rejection sampling
+ *                      PAPER.md:L54 (sec. 2.2), L445 (sec. D.1: accept / resample at the first rejection from
+ *                      the adjusted target distribution / bonus token), L544 (needs the full distribution)
+ *
+ * Conventions (every entry point):
+ *   - Every data pointer is a caller-owned DEVICE pointer unless the comment says "host".  The library
+ *     allocates no device memory and keeps no device state.
+ *   - All work is enqueued on `stream` (a cudaStream_t passed as void*; NULL = legacy default stream).
+ *     No call synchronises.  Outputs are valid once the stream reaches the end of the call.
+ *     Calls are CUDA-graph capturable.
+ *   - Errors: the return code only (no exceptions, no abort, no printing).  Arguments are validated before
+ *     anything is launched; on error nothing is enqueued.  There is NO CPU fallback: on a device that is
+ *     not sm_100 the compute calls return ER_ERR_ARCH.
+ *   - Determinism: identical inputs give bit-identical outputs (fixed split-K reduction order, no
+ *     floating-point atomics).
+ *
+ * Data layouts:
+ *   W        bf16 [N][K], row-major, K contiguous, row stride ldw elements (torch nn.Linear.weight)
+ *   qweight  uint32 [N][K/8] row-major ("ER_PACK_V1"): word (n, j) holds the 8 codes of logical
+ *            k = 8 j + pi[i] in bits [4 i, 4 i + 4), pi = (0,2,4,6,1,3,5,7); stored nibble u = q + 8,
+ *            q in [-8, 7].  So (word >> 4 t) & 0x000F000F is the pair (k = 8 j + 2 t, 8 j + 2 t + 1).
+ *   scales   bf16 [K/128][N] (group-major, N contiguous); s = bf16_rne(max|w| / 7) per 128 consecutive k
+ *   X        bf16 [M][K], row stride ldx elements
+ *   Y        bf16 or fp32 [M][N], row stride ldy elements
+ */
+#ifndef ER_H_
+#define ER_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ER_ABI_VERSION 1
+#define ER_GROUP 128
+
+typedef enum {
+  ER_OK = 0,
+  ER_ERR_NULL = 1,      /* a required pointer is NULL */
+  ER_ERR_SHAPE = 2,     /* a size is out of the supported range (see each call) */
+  ER_ERR_ALIGN = 3,     /* a pointer or leading dimension violates the stated alignment */
+  ER_ERR_DTYPE = 4,     /* unsupported dtype / input-form combination */
+  ER_ERR_WORKSPACE = 5, /* workspace missing or smaller than er_gemm_workspace_bytes() */
+  ER_ERR_ARCH = 6,      /* current device is not compute capability 10.x */
+  ER_ERR_CUDA = 7       /* a CUDA runtime/driver call failed; see er_last_cuda_error() */
+} er_status;
+
+typedef enum { ER_BF16 = 0, ER_F32 = 1 } er_dtype;
+
+/* Static, never-freed description of a status code. */
+const char* er_status_str(int status);
+/* Thread-local cudaError_t (as int) behind the last ER_ERR_CUDA returned on this thread; 0 if none. */
+int er_last_cuda_error(void);
+int er_abi_version(void);
+
+/* Sizes in bytes of the refresh outputs for a [N][K] weight.  0 if the shape is unsupported. */
+size_t er_packed_bytes(int64_t N, int64_t K);            /* N*K/2 */
+size_t er_scales_bytes(int64_t N, int64_t K, int group); /* (K/group)*N*2 */
+/* Workspace er_w4a16_gemm needs for this problem (split-K partials + tile counters).  Never 0 for a
+ * valid shape.  The first ER_GEMM_COUNTER_BYTES of the workspace hold tile counters that MUST be zero
+ * before the first call that uses the workspace (er_gemm_workspace_init does that); every call leaves
+ * them zero again, so one workspace may be reused by any number of calls on one stream. */
+size_t er_gemm_workspace_bytes(int64_t M, int64_t N, int64_t K);
+#define ER_GEMM_COUNTER_BYTES 16384
+int er_gemm_workspace_init(void* workspace, size_t workspace_bytes, void* stream);
+
+/* (2) Drafter refresh: quantize + pack one linear weight.
+ *   w_bf16      [N][K] bf16, row stride ldw_elems (>= K); base 16-byte aligned, ldw_elems % 8 == 0
+ *   group       must be 128 (ER_GROUP); K % 128 == 0, N >= 1
+ *   qweight_out uint32 [N][K/8]   (er_packed_bytes), 16-byte aligned
+ *   scales_out  bf16 [K/128][N]   (er_scales_bytes), 2-byte aligned
+ * Per group of 128 consecutive k of a row: amax = max|w|; s = bf16_rne(amax / 7) (IEEE fp32 divide);
+ * q = clamp(rint(w / s), -8, 7) (ties to even, divide by the ROUNDED scale); s == 0 -> q = 0, s = +0.
+ * NaN/Inf weights are outside the contract (no fault, unspecified codes). */
+int er_quantize_pack(const void* w_bf16, int64_t N, int64_t K, int64_t ldw_elems, int group,
+                     void* qweight_out, void* scales_out, void* stream);
+
+/* (1) Drafter linear:  Y[m][n] = sum_k X[m][k] * q[n][k] * s[k/128][n].
+ *   x_bf16   [M][K] bf16, row stride ldx_elems; base 16-byte aligned, ldx_elems % 8 == 0; M >= 1
+ *   qweight, scales  as produced by er_quantize_pack (any nibble incl. -8 is legal); N % 128 == 0,
+ *            K % 128 == 0, group == 128; qweight 16-byte aligned, scales 16-byte aligned
+ *   y        [M][N] of y_dtype (ER_BF16: fp32 accumulator rounded RNE; ER_F32: the accumulator itself),
+ *            row stride ldy_elems; rows >= M are never written
+ *   workspace  caller-provided, >= er_gemm_workspace_bytes(M,N,K), 16-byte aligned, counters zeroed once
+ * Arithmetic: codes are widened exactly to bf16, contracted with X on the tensor cores with fp32
+ * accumulation per 128-k group, each group's partial sum multiplied by its fp32 scale and added in fp32
+ * (no rounding of q*s), split-K partials reduced in ascending split order. */
+int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems,
+                  const void* qweight, const void* scales, int64_t N, int group,
+                  void* y, int64_t ldy_elems, int y_dtype,
+                  void* workspace, size_t workspace_bytes, void* stream);
+
+/* Same contract and results up to fp32 summation order, computed by a plain CUDA-core kernel (no TMA, no
+ * tensor cores).  Debug / cross-check aid, not a timed path; needs no workspace. */
+int er_w4a16_gemm_simt(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems,
+                       const void* qweight, const void* scales, int64_t N, int group,
+                       void* y, int64_t ldy_elems, int y_dtype, void* stream);
+
+/* (3) Speculative-decoding verification, one result per sequence b < B.
+ *   target  [B][gamma+1][V]  (row gamma = bonus position), draft [B][gamma][V]; contiguous, 16-byte aligned
+ *   in_dtype / inputs_are_logits: (ER_F32, 0) = fp32 probabilities; (ER_BF16, 1) and (ER_F32, 1) = logits,
+ *            softmax(logit / temperature) is computed in fp32 inside the kernel; (ER_BF16, 0) -> ER_ERR_DTYPE
+ *   temperature > 0 (used only for logits)
+ *   draft_tokens int32 [B][gamma] in [0, V) (out-of-range ids are clamped for reads)
+ *   u_accept fp32 [B][gamma] in [0,1);  u_sample fp32 [B] in [0,1)
+ *   1 <= gamma <= 16, B >= 0 (B == 0 is a no-op), 1 <= V <= 2^20
+ *   accept_count int32 [B] out: n = number of leading i with  fp32(u_i * q_i(x_i)) < p_i(x_i)
+ *   out_tokens   int32 [B][gamma+1] out: x_1..x_n, then the token drawn at position n+1 by inverse CDF
+ *            (vocab order, token = min{v : C(v) > u_sample * R}) from w = max(0, p_{n+1} - q_{n+1})
+ *            (n < gamma; w = p_{n+1} if that residual is identically 0) or w = p_{gamma+1} (n == gamma),
+ *            then -1 padding. */
+int er_spec_verify(const void* target, const void* draft, int in_dtype, int inputs_are_logits,
+                   float temperature, const int32_t* draft_tokens, const float* u_accept,
+                   const float* u_sample, int32_t B, int32_t gamma, int32_t V,
+                   int32_t* accept_count, int32_t* out_tokens, void* stream);
+
+/* Parity helper: qweight uint32 [N][K/8] -> int8 codes [N][K] in [-8, 7] (device). Not timed. */
+int er_unpack_codes(const void* qweight, int64_t N, int64_t K, int8_t* codes_out, void* stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ER_H_ */

@@ -1,0 +1,172 @@
+"""Thin ctypes binding over liber_b200.so (include/er.h).  Argument marshalling only: every step of the
+path runs in the CUDA kernels behind the C ABI.  PyTorch supplies device memory and streams.
+
+There is no CPU fallback: if the library is missing it is built with nvcc (in-tree); if that fails, or a
+call returns a non-zero status, an exception is raised.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+from . import build as _build
+
+ER_BF16, ER_F32 = 0, 1
+GROUP = 128
+COUNTER_BYTES = 16384
+
+_lib = None
+
+
+class ErError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        lib = load()
+        msg = lib.er_status_str(status).decode()
+        cuda = lib.er_last_cuda_error() if status == 7 else 0
+        super().__init__(f"{where}: {msg}" + (f" (cudaError {cuda})" if cuda else ""))
+        self.status = status
+
+
+def load() -> ctypes.CDLL:
+    """Load (building first if stale/missing) the C-ABI library.  Raises if it cannot be had."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB_PATH
+    if not os.path.exists(path) or (os.environ.get("ER_REBUILD") == "1"):
+        path = _build.build_library()
+    lib = ctypes.CDLL(path)
+    vp, i64, i32, sz, f32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_size_t, ctypes.c_float
+    lib.er_status_str.restype = ctypes.c_char_p
+    lib.er_status_str.argtypes = [ctypes.c_int]
+    lib.er_last_cuda_error.restype = ctypes.c_int
+    lib.er_abi_version.restype = ctypes.c_int
+    lib.er_packed_bytes.restype = sz
+    lib.er_packed_bytes.argtypes = [i64, i64]
+    lib.er_scales_bytes.restype = sz
+    lib.er_scales_bytes.argtypes = [i64, i64, ctypes.c_int]
+    lib.er_gemm_workspace_bytes.restype = sz
+    lib.er_gemm_workspace_bytes.argtypes = [i64, i64, i64]
+    lib.er_gemm_workspace_init.restype = ctypes.c_int
+    lib.er_gemm_workspace_init.argtypes = [vp, sz, vp]
+    lib.er_quantize_pack.restype = ctypes.c_int
+    lib.er_quantize_pack.argtypes = [vp, i64, i64, i64, ctypes.c_int, vp, vp, vp]
+    lib.er_w4a16_gemm.restype = ctypes.c_int
+    lib.er_w4a16_gemm.argtypes = [vp, i64, i64, i64, vp, vp, i64, ctypes.c_int, vp, i64, ctypes.c_int, vp, sz, vp]
+    lib.er_w4a16_gemm_simt.restype = ctypes.c_int
+    lib.er_w4a16_gemm_simt.argtypes = [vp, i64, i64, i64, vp, vp, i64, ctypes.c_int, vp, i64, ctypes.c_int, vp]
+    lib.er_spec_verify.restype = ctypes.c_int
+    lib.er_spec_verify.argtypes = [vp, vp, ctypes.c_int, ctypes.c_int, f32, vp, vp, vp, i32, i32, i32, vp, vp, vp]
+    lib.er_unpack_codes.restype = ctypes.c_int
+    lib.er_unpack_codes.argtypes = [vp, i64, i64, vp, vp]
+    lib.er_gemm_tuning.restype = ctypes.c_int
+    lib.er_gemm_tuning.argtypes = [ctypes.c_int, ctypes.c_int]
+    if lib.er_abi_version() != 1:
+        raise RuntimeError("liber_b200.so ABI version mismatch")
+    _lib = lib
+    return lib
+
+
+def _stream(t: torch.Tensor) -> int:
+    return torch.cuda.current_stream(t.device).cuda_stream
+
+
+def _check(status: int, where: str):
+    if status != 0:
+        raise ErError(status, where)
+
+
+def _cuda(t: torch.Tensor, name: str):
+    if not t.is_cuda:
+        raise ValueError(f"{name} must be a CUDA tensor (the library takes device pointers; no CPU path exists)")
+
+
+def packed_bytes(N: int, K: int) -> int:
+    return load().er_packed_bytes(N, K)
+
+
+def scales_bytes(N: int, K: int, group: int = GROUP) -> int:
+    return load().er_scales_bytes(N, K, group)
+
+
+def gemm_workspace_bytes(M: int, N: int, K: int) -> int:
+    return load().er_gemm_workspace_bytes(M, N, K)
+
+
+def gemm_workspace(M: int, N: int, K: int, device) -> torch.Tensor:
+    """Allocate and initialise (counters zeroed) a workspace large enough for this problem."""
+    nbytes = gemm_workspace_bytes(M, N, K)
+    if nbytes == 0:
+        raise ErError(2, "er_gemm_workspace_bytes")
+    ws = torch.empty(nbytes, dtype=torch.uint8, device=device)
+    _check(load().er_gemm_workspace_init(ws.data_ptr(), nbytes, _stream(ws)), "er_gemm_workspace_init")
+    return ws
+
+
+def quantize_pack(w: torch.Tensor, qweight: torch.Tensor | None = None, scales: torch.Tensor | None = None,
+                  group: int = GROUP):
+    """bf16 W[N][K] -> (qweight int32 [N][K/8] (ER_PACK_V1 bits), scales bf16 [K/128][N])."""
+    _cuda(w, "w")
+    assert w.dtype == torch.bfloat16 and w.dim() == 2 and w.stride(1) == 1
+    N, K = w.shape
+    if qweight is None:
+        qweight = torch.empty((N, K // 8), dtype=torch.int32, device=w.device)
+    if scales is None:
+        scales = torch.empty((K // group, N), dtype=torch.bfloat16, device=w.device)
+    _check(load().er_quantize_pack(w.data_ptr(), N, K, w.stride(0), group, qweight.data_ptr(), scales.data_ptr(),
+                                   _stream(w)), "er_quantize_pack")
+    return qweight, scales
+
+
+def w4a16_gemm(x: torch.Tensor, qweight: torch.Tensor, scales: torch.Tensor, out_dtype=torch.bfloat16,
+               y: torch.Tensor | None = None, workspace: torch.Tensor | None = None, simt: bool = False):
+    """Y[M][N] = X[M][K] . dequant(qweight, scales)[N][K]^T."""
+    _cuda(x, "x")
+    assert x.dtype == torch.bfloat16 and x.dim() == 2 and x.stride(1) == 1
+    M, K = x.shape
+    N = qweight.shape[0]
+    if y is None:
+        y = torch.empty((M, N), dtype=out_dtype, device=x.device)
+    ydt = ER_F32 if y.dtype == torch.float32 else ER_BF16
+    lib = load()
+    if simt:
+        _check(lib.er_w4a16_gemm_simt(x.data_ptr(), M, K, x.stride(0), qweight.data_ptr(), scales.data_ptr(), N, GROUP,
+                                      y.data_ptr(), y.stride(0), ydt, _stream(x)), "er_w4a16_gemm_simt")
+        return y
+    if workspace is None:
+        workspace = gemm_workspace(M, N, K, x.device)
+    _check(lib.er_w4a16_gemm(x.data_ptr(), M, K, x.stride(0), qweight.data_ptr(), scales.data_ptr(), N, GROUP,
+                             y.data_ptr(), y.stride(0), ydt, workspace.data_ptr(), workspace.numel(), _stream(x)),
+           "er_w4a16_gemm")
+    return y
+
+
+def spec_verify(target: torch.Tensor, draft: torch.Tensor, draft_tokens: torch.Tensor, u_accept: torch.Tensor,
+                u_sample: torch.Tensor, inputs_are_logits: bool, temperature: float = 1.0,
+                accept_count: torch.Tensor | None = None, out_tokens: torch.Tensor | None = None):
+    """target [B][gamma+1][V], draft [B][gamma][V] -> (accept_count int32 [B], out_tokens int32 [B][gamma+1])."""
+    _cuda(target, "target")
+    B, G1, V = target.shape
+    gamma = G1 - 1
+    assert draft.shape == (B, gamma, V) and target.is_contiguous() and draft.is_contiguous()
+    assert target.dtype == draft.dtype and target.dtype in (torch.float32, torch.bfloat16)
+    assert draft_tokens.dtype == torch.int32 and u_accept.dtype == torch.float32 and u_sample.dtype == torch.float32
+    dt = ER_F32 if target.dtype == torch.float32 else ER_BF16
+    if accept_count is None:
+        accept_count = torch.empty((B,), dtype=torch.int32, device=target.device)
+    if out_tokens is None:
+        out_tokens = torch.empty((B, gamma + 1), dtype=torch.int32, device=target.device)
+    _check(load().er_spec_verify(target.data_ptr(), draft.data_ptr(), dt, int(inputs_are_logits), float(temperature),
+                                 draft_tokens.data_ptr(), u_accept.data_ptr(), u_sample.data_ptr(), B, gamma, V,
+                                 accept_count.data_ptr(), out_tokens.data_ptr(), _stream(target)), "er_spec_verify")
+    return accept_count, out_tokens
+
+
+def unpack_codes(qweight: torch.Tensor) -> torch.Tensor:
+    _cuda(qweight, "qweight")
+    N, J = qweight.shape
+    codes = torch.empty((N, J * 8), dtype=torch.int8, device=qweight.device)
+    _check(load().er_unpack_codes(qweight.data_ptr(), N, J * 8, codes.data_ptr(), _stream(qweight)), "er_unpack_codes")
+    return codes

@@ -1,0 +1,85 @@
+"""GPU parity: er_quantize_pack / er_unpack_codes vs the oracle, bit-exact (Q1-Q12)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import er_oracle as O
+from paper_2606_18967_b200 import er, inputs as I
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+def _check_exact(w):
+    qw, sc = er.quantize_pack(w)
+    torch.cuda.synchronize()
+    qw_ref, sc_ref = O.quantize_pack(I.as_u16(w))
+    qw_np = qw.cpu().numpy().view(np.uint32)
+    sc_np = I.as_u16(sc)
+    assert np.array_equal(sc_np, sc_ref), f"scale mismatches: {(sc_np != sc_ref).sum()}"
+    assert np.array_equal(qw_np, qw_ref), f"packed word mismatches: {(qw_np != qw_ref).sum()}"
+    return qw, sc
+
+
+def test_config0_whole_matrix_bit_exact():
+    w = I.weight_bf16(2048, 2048, I.seed_of("cfg0", "w"), device=DEV)
+    qw, _ = _check_exact(w)
+    codes = er.unpack_codes(qw).cpu().numpy()
+    assert np.array_equal(codes, O.unpack_codes(qw.cpu().numpy().view(np.uint32)))
+    assert codes.min() >= -7 and codes.max() == 7
+
+
+@pytest.mark.parametrize("N,K", [(1, 128), (33, 384), (130, 1152), (257, 640), (96, 4096)])
+def test_ragged_shapes_bit_exact(N, K):
+    w = I.weight_bf16(N, K, I.seed_of("ragged", N, K), device=DEV, outlier_frac=0.001)
+    _check_exact(w)
+
+
+def test_outliers_and_ties_bit_exact():
+    # config-3 value structure: 0.1 % outliers at 20x; ~0.24 % of quotients are exact ties
+    w = I.weight_bf16(1024, 3584, I.seed_of("cfg3", "layer0", "o"), device=DEV, outlier_frac=0.001)
+    _check_exact(w)
+
+
+def test_strided_input_and_special_groups():
+    base = I.weight_bf16(64, 1024, 7, device=DEV)
+    w = base[:, :512]                       # ldw = 1024 > K = 512
+    assert w.stride(0) == 1024
+    qw, sc = er.quantize_pack(w)
+    qr, sr = O.quantize_pack(I.as_u16(w.contiguous()))
+    assert np.array_equal(qw.cpu().numpy().view(np.uint32), qr) and np.array_equal(I.as_u16(sc), sr)
+    z = torch.zeros((32, 256), dtype=torch.bfloat16, device=DEV)
+    z[0, :128] = 1.0                        # a group of equal values; other groups all zero (Q8)
+    z[1, 130] = -3.0
+    z[2, 0] = 1e-38                         # denormal-range scale
+    z[2, 1] = 4e-39
+    _check_exact(z)
+
+
+def test_exhaustive_bf16_values_against_fixed_scales():
+    # every finite bf16 value as w, against a handful of group maxima (brute force over 2^16 values)
+    u = np.arange(65536, dtype=np.uint16)
+    f = O.bf16_to_f32(u)
+    for amax_bits in (0x3F80, 0x3C23, 0x4110, 0x3DCC, 0x3FFF):
+        amax = float(O.bf16_to_f32(np.uint16(amax_bits)))
+        keep = np.isfinite(f) & (np.abs(f) <= amax)
+        vals = u[keep]
+        pad = (-len(vals)) % 127
+        vals = np.concatenate([vals, np.zeros(pad, dtype=np.uint16)])
+        rows = vals.reshape(-1, 127)
+        full = np.concatenate([np.full((rows.shape[0], 1), amax_bits, dtype=np.uint16), rows], axis=1)
+        w = I.from_u16(full, DEV)
+        _check_exact(w)
+
+
+def test_sampled_groups_of_a_7b_layer():
+    # config 3: 1 % of groups of a large tensor checked against the oracle on the sampled rows only
+    N, K = 4608, 3584
+    w = I.weight_bf16(N, K, I.seed_of("cfg3", 5, "qkv"), device=DEV, outlier_frac=0.001)
+    qw, sc = er.quantize_pack(w)
+    rng = np.random.default_rng(5)
+    rows = np.sort(rng.choice(N, size=N // 100, replace=False))
+    wr = I.as_u16(w[torch.from_numpy(rows).to(DEV)])
+    qr, sr = O.quantize_pack(wr)
+    assert np.array_equal(qw.cpu().numpy().view(np.uint32)[rows], qr)
+    assert np.array_equal(I.as_u16(sc)[:, rows], sr)

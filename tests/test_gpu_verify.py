@@ -1,0 +1,127 @@
+"""GPU parity: er_spec_verify vs the oracle (V1-V12): accept counts and accepted-prefix tokens
+exact, -1 padding exact, final token by rule V10 (exact, or inside its own fp64 CDF interval +-1e-5)."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import er_oracle as O
+from paper_2606_18967_b200 import er, inputs as I
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+def _run_and_check(tgt, drf, toks, ua, us, logits, dtype, temperature=1.0, min_margin=1e-5):
+    """tgt/drf: float32 numpy (probs or logits).  dtype: torch dtype sent to the device."""
+    t_dev = torch.from_numpy(tgt).to(DEV).to(dtype).contiguous()
+    d_dev = torch.from_numpy(drf).to(DEV).to(dtype).contiguous()
+    # the oracle sees exactly the values the device sees
+    t_host = t_dev.float().cpu().numpy()
+    d_host = d_dev.float().cpu().numpy()
+    acc, out = er.spec_verify(t_dev, d_dev, torch.from_numpy(toks).to(DEV), torch.from_numpy(ua).to(DEV),
+                              torch.from_numpy(us).to(DEV), logits, temperature)
+    torch.cuda.synchronize()
+    acc, out = acc.cpu().numpy(), out.cpu().numpy()
+    acc_ref, out_ref, diag = O.spec_verify(t_host, d_host, toks, ua, us, inputs_are_logits=logits,
+                                           temperature=temperature, return_diag=True)
+    B, G1 = out.shape
+    thin = [m for d in diag for m in d["margins"] if m < min_margin]
+    assert not thin, f"accept tests with margin < {min_margin}: {thin} (listed, never re-seeded)"
+    assert np.array_equal(acc, acc_ref)
+    n_exact = 0
+    for b in range(B):
+        n = int(acc_ref[b])
+        assert np.array_equal(out[b, :n], out_ref[b, :n])
+        assert np.all(out[b, n + 1:] == -1)
+        if out[b, n] == out_ref[b, n]:
+            n_exact += 1
+        else:
+            assert O.token_in_widened_interval(diag[b], int(out[b, n])), (b, out[b, n], out_ref[b, n])
+    return acc, out, n_exact
+
+
+def _softmax(x):
+    return O.softmax64(x).astype(np.float32)
+
+
+def test_config0_probs_fp32():
+    B, gamma, V = 4, 4, 32000
+    lt, ld = I.verify_logits_f32(B, gamma, V, I.seed_of("cfg0", "verify"))
+    p, q = _softmax(lt), _softmax(ld)
+    toks = I.sample_draft_tokens(q, I.seed_of("cfg0", "x"))
+    ua = I.uniforms((B, gamma), I.seed_of("cfg0", "ua"))
+    us = I.uniforms((B,), I.seed_of("cfg0", "us"))
+    _run_and_check(p, q, toks, ua, us, False, torch.float32)
+
+
+def test_q_equals_p_accepts_everything():
+    B, gamma, V = 3, 5, 5000
+    lt, _ = I.verify_logits_f32(B, gamma, V, 11)
+    p = _softmax(lt)
+    q = p[:, :gamma].copy()
+    toks = I.sample_draft_tokens(q, 12)
+    ua = I.uniforms((B, gamma), 13)
+    us = I.uniforms((B,), 14)
+    acc, out, _ = _run_and_check(p, q, toks, ua, us, False, torch.float32, min_margin=0.0)
+    assert np.all(acc == gamma) and np.all(out[:, gamma] >= 0)
+
+
+@pytest.mark.parametrize("V", [1, 7, 255, 8192, 8193, 20011])
+def test_ragged_vocab_sizes_logits_f32(V):
+    B, gamma = 5, 3
+    lt, ld = I.verify_logits_f32(B, gamma, V, I.seed_of("ragged", V), draft_noise=0.5)
+    toks = I.sample_draft_tokens(_softmax(ld), V + 1)
+    ua = I.uniforms((B, gamma), V + 2)
+    us = I.uniforms((B,), V + 3)
+    _run_and_check(lt, ld, toks, ua, us, True, torch.float32)
+
+
+def test_forced_rejection_and_zero_probability():
+    # p(x_1) = 0 -> rejected at once and the resampled token differs from x_1; one-hot p on x -> accepted
+    B, gamma, V = 2, 2, 64
+    p = np.full((B, gamma + 1, V), 1.0 / (V - 1), dtype=np.float32)
+    q = np.full((B, gamma, V), 1.0 / V, dtype=np.float32)
+    toks = np.array([[3, 4], [5, 6]], dtype=np.int32)
+    p[0, 0, 3] = 0.0
+    p[1, :, :] = 0.0
+    p[1, 0, 5] = 1.0
+    p[1, 1, 6] = 1.0
+    p[1, 2, 9] = 1.0
+    ua = np.full((B, gamma), 0.999, dtype=np.float32)
+    us = np.array([0.5, 0.5], dtype=np.float32)
+    acc, out, _ = _run_and_check(p, q, toks, ua, us, False, torch.float32, min_margin=0.0)
+    assert acc[0] == 0 and out[0, 0] != 3
+    assert acc[1] == 2 and out[1, 2] == 9
+
+
+@pytest.mark.parametrize("gamma", [2, 4, 8])
+def test_config4_bf16_logits(gamma):
+    B, V = 8, 152064          # config 4 shape at a batch the oracle finishes in seconds
+    lt, ld = I.verify_logits_f32(B, gamma, V, I.seed_of("cfg4", gamma), draft_noise=0.5)
+    t_b = torch.from_numpy(lt).to(torch.bfloat16).float().numpy()
+    d_b = torch.from_numpy(ld).to(torch.bfloat16).float().numpy()
+    toks = I.sample_draft_tokens(_softmax(d_b), I.seed_of("cfg4", "x", gamma))
+    ua = I.uniforms((B, gamma), I.seed_of("cfg4", "ua", gamma))
+    us = I.uniforms((B,), I.seed_of("cfg4", "us", gamma))
+    acc, out, n_exact = _run_and_check(t_b, d_b, toks, ua, us, True, torch.bfloat16)
+    assert n_exact >= B // 2   # most tokens are exactly the oracle's; the rest passed the V10 window
+
+
+def test_temperature():
+    B, gamma, V = 4, 3, 4096
+    lt, ld = I.verify_logits_f32(B, gamma, V, 77, draft_noise=0.5)
+    toks = I.sample_draft_tokens(O.softmax64(ld, 0.6).astype(np.float32), 78)
+    _run_and_check(lt, ld, toks, I.uniforms((B, gamma), 79), I.uniforms((B,), 80), True, torch.float32, temperature=0.6)
+
+
+def test_deterministic():
+    B, gamma, V = 4, 4, 32000
+    lt, ld = I.verify_logits_f32(B, gamma, V, 5, draft_noise=0.5)
+    t = torch.from_numpy(lt).to(DEV).to(torch.bfloat16)
+    d = torch.from_numpy(ld).to(DEV).to(torch.bfloat16)
+    toks = torch.from_numpy(I.sample_draft_tokens(_softmax(ld), 6)).to(DEV)
+    ua = torch.from_numpy(I.uniforms((B, gamma), 7)).to(DEV)
+    us = torch.from_numpy(I.uniforms((B,), 8)).to(DEV)
+    a1, o1 = er.spec_verify(t, d, toks, ua, us, True)
+    a2, o2 = er.spec_verify(t, d, toks, ua, us, True)
+    assert torch.equal(a1, a2) and torch.equal(o1, o2)
