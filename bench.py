@@ -1,0 +1,520 @@
+#!/usr/bin/env python
+"""bench.py -- the headline measurement of BASELINE.json ("W4A16 drafter GEMM HBM GB/s & % of peak vs batch
+1-256; refresh GB/s; verify us") on config 1 (the linear set of one 7B decoder layer) plus config 4's verify.
+
+One STEP = one pass of the whole hot path over one batch of synthetic input:
+  refresh   er_quantize_pack of the four linears of one 7B layer                      (4 launches)
+  gemm      er_w4a16_gemm of QKV, O, gate/up, down at every M in {1,...,256}          (36 launches)
+  verify    er_spec_verify at B=64, gamma=4, V=152064, bf16 logits                    (1 launch)
+The step is captured in CUDA graphs (one per weight-rotation phase: four distinct layer copies, 470 MB
+packed, so that no GEMM re-reads L2-hot weights) with external timing events around every launch; the
+per-launch durations of the timed region come from those events.
+
+`value` = algorithmic GEMM bytes at M <= 16 (the memory-bound regime the north_star targets) / their time.
+`python bench.py --impl reference` times the CPU oracle on a bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "w4a16_drafter_gemm_hbm_gbs_m<=16 (7B layer; +vs-M table, refresh GB/s, verify us in detail)"
+UNIT = "GB/s"
+NOMINAL_HBM_GBS = 8000.0          # BASELINE.json "~8 TB/s" (context)
+FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+W4_BYTES_PER_WEIGHT = 0.5 + 2.0 / 128.0
+REFRESH_BYTES_PER_ELEM = 2.0 + W4_BYTES_PER_WEIGHT
+LAYER_COPIES = 4
+VERIFY_B, VERIFY_GAMMA, VERIFY_V = 64, 4, 152064
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (w4a16_gemm_kernel<16>,
+# gate_up at M=16) from the ncu --set full capture summarised in profiles/; None until captured.
+NCU_TRAFFIC_BYTES = None
+
+
+def log(*a):
+    print(*a, file=sys.stderr, flush=True)
+
+
+def gemm_bytes(M, N, K):
+    return W4_BYTES_PER_WEIGHT * N * K + 2.0 * M * K + 2.0 * M * N
+
+
+def hbm_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+# ------------------------------------------------------------------------------------------------------
+# clocks: NVML samples taken DURING the timed region
+# ------------------------------------------------------------------------------------------------------
+class ClockSampler:
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting",
+               0x10: "sync_boost"}
+
+    def __init__(self, torch_device_index):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop = threading.Event()
+        self._thread = None
+        self.h = None
+        try:
+            import pynvml
+            import torch
+            self.nv = pynvml
+            pynvml.nvmlInit()
+            uuid = str(torch.cuda.get_device_properties(torch_device_index).uuid)
+            if not uuid.startswith("GPU-"):
+                uuid = "GPU-" + uuid
+            try:
+                self.h = pynvml.nvmlDeviceGetHandleByUUID(uuid)
+            except Exception:
+                self.h = pynvml.nvmlDeviceGetHandleByIndex(torch_device_index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception as e:  # no NVML: clocks unknown, say so
+            log(f"[bench] NVML unavailable: {e}")
+
+    def _loop(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                try:
+                    r = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.001)
+
+    def start(self):
+        if self.h is not None:
+            self._thread = threading.Thread(target=self._loop, daemon=True)
+            self._thread.start()
+
+    def stop(self):
+        if self._thread is not None:
+            self._stop.set()
+            self._thread.join()
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz, "samples": len(s),
+                "reasons": sorted(self.reasons)}
+
+
+# ------------------------------------------------------------------------------------------------------
+# CPU oracle legs (cpu_baseline of the product line; the whole --impl reference arm)
+# ------------------------------------------------------------------------------------------------------
+def oracle_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+    except Exception:
+        n = 1
+    return int(min(n, len(os.sched_getaffinity(0))))
+
+
+class OracleSample:
+    """A bounded sample of the step for the CPU oracle, as it stands (never tuned): refresh of the O
+    projection [3584x3584], its W4A16 linear at M in {1, 16}, and verify of `vb` sequences of the step's
+    verify workload (gamma=4, V=152064, bf16 logits).  Inputs are generated once, outside the timing."""
+
+    def __init__(self, vb=1):
+        import numpy as np
+        import torch
+        from paper_2606_18967_b200 import inputs as I
+        self.np, self.I = np, I
+        self.N, self.K = 3584, 3584
+        self.w = I.as_u16(I.weight_bf16(self.N, self.K, I.seed_of("bench", 0, "o"), device="cpu"))
+        self.x = {M: I.as_u16(I.activation_bf16(M, self.K, I.seed_of("bench", "x", M, self.K), device="cpu"))
+                  for M in (1, 16)}
+        tgt, drf = I.verify_logits_bf16_device(vb, VERIFY_GAMMA, VERIFY_V, I.seed_of("bench", "verify"), "cpu")
+        self.toks = I.sample_draft_tokens_gumbel(drf, I.seed_of("bench", "tok")).numpy()
+        self.tgt, self.drf = tgt.float().numpy(), drf.float().numpy()
+        self.ua = I.uniforms((vb, VERIFY_GAMMA), 1)
+        self.us = I.uniforms((vb,), 2)
+        self.vb = vb
+        self.describe = (f"refresh O-proj 3584x3584; W4A16 linear O-proj at M in {{1,16}}; verify {vb} seq "
+                         f"(gamma={VERIFY_GAMMA}, V={VERIFY_V}, bf16 logits)")
+
+    def step(self):
+        from oracle import er_oracle as O
+        t0 = time.perf_counter()
+        qw, sc = O.quantize_pack(self.w)
+        t1 = time.perf_counter()
+        for M in (1, 16):
+            O.w4a16_gemm(self.x[M], qw, sc)
+        t2 = time.perf_counter()
+        O.spec_verify(self.tgt, self.drf, self.toks, self.ua, self.us, inputs_are_logits=True)
+        t3 = time.perf_counter()
+        return t1 - t0, t2 - t1, t3 - t2
+
+    def rates(self, tq, tg, tv):
+        gb = sum(gemm_bytes(M, self.N, self.K) for M in (1, 16)) / 1e9
+        return {"gemm_gbs": gb / tg, "refresh_gbs": REFRESH_BYTES_PER_ELEM * self.N * self.K / 1e9 / tq,
+                "verify_us_per_seq": tv / self.vb * 1e6}
+
+
+def cpu_baseline_leg(budget_s=15.0):
+    smp = OracleSample(vb=1)
+    smp.step()  # warm-up (page-in, BLAS thread start)
+    acc, n, t_start = [0.0, 0.0, 0.0], 0, time.perf_counter()
+    while n < 1 or (time.perf_counter() - t_start) < budget_s:
+        for i, t in enumerate(smp.step()):
+            acc[i] += t
+        n += 1
+    r = smp.rates(acc[0] / n, acc[1] / n, acc[2] / n)
+    return {"value": round(r["gemm_gbs"], 4), "unit": UNIT, "cores": oracle_threads(), "kind": "oracle",
+            "sample": f"{n} x [{smp.describe}]", "refresh_gbs": round(r["refresh_gbs"], 4),
+            "verify_us_per_seq": round(r["verify_us_per_seq"], 1)}
+
+
+def reference_arm(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    smp = OracleSample(vb=1)
+    for _ in range(args.warmup):
+        smp.step()
+    acc = [0.0, 0.0, 0.0]
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        for i, t in enumerate(smp.step()):
+            acc[i] += t
+    total = time.perf_counter() - t0
+    K = max(args.steps, 1)
+    r = smp.rates(acc[0] / K, acc[1] / K, acc[2] / K)
+    val = round(r["gemm_gbs"], 4)
+    cores = oracle_threads()
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": round(total / K * 1e3, 3),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "config1: 7B decoder-layer linear set (bounded oracle sample per step)",
+                       "sample": smp.describe},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": smp.describe,
+                             "refresh_gbs": round(r["refresh_gbs"], 4),
+                             "verify_us_per_seq": round(r["verify_us_per_seq"], 1)},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------------------
+# product arm
+# ------------------------------------------------------------------------------------------------------
+def product_arm(args):
+    import torch
+    from paper_2606_18967_b200 import er, inputs as I
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback (use --impl reference "
+                         "for the oracle arm)")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist_
+        dist = dist_
+        dist.init_process_group("nccl", device_id=dev)
+    er.load()
+
+    shape = I.SHAPE_7B
+    linears = shape.linears()                      # (name, N, K)
+    Ms = list(I.M_SWEEP)
+    L = LAYER_COPIES
+
+    # ---- resident inputs (HBM) ----------------------------------------------------------------------
+    src = [{n: I.weight_bf16(N, K, I.seed_of("bench", c, n), device=dev) for n, N, K in linears} for c in range(L)]
+    qw = [{n: torch.empty((N, K // 8), dtype=torch.int32, device=dev) for n, N, K in linears} for _ in range(L)]
+    sc = [{n: torch.empty((K // 128, N), dtype=torch.bfloat16, device=dev) for n, N, K in linears} for _ in range(L)]
+    for c in range(L):
+        for n, N, K in linears:
+            er.quantize_pack(src[c][n], qw[c][n], sc[c][n])
+    Ks = sorted({K for _, _, K in linears})
+    X = {(M, K): I.activation_bf16(M, K, I.seed_of("bench", "x", M, K), device=dev) for M in Ms for K in Ks}
+    Y = {n: torch.empty((max(Ms), N), dtype=torch.bfloat16, device=dev) for n, N, K in linears}
+    ws_bytes = max(er.gemm_workspace_bytes(M, N, K) for M in Ms for _, N, K in linears)
+    ws = torch.empty(ws_bytes, dtype=torch.uint8, device=dev)
+    er._check(er.load().er_gemm_workspace_init(ws.data_ptr(), ws_bytes, torch.cuda.current_stream().cuda_stream),
+              "er_gemm_workspace_init")
+    B, G, V = VERIFY_B, VERIFY_GAMMA, VERIFY_V
+    v_tgt, v_drf = I.verify_logits_bf16_device(B, G, V, I.seed_of("bench", "verify"), dev)
+    v_tok = I.sample_draft_tokens_gumbel(v_drf, I.seed_of("bench", "tok"))
+    v_ua = I.uniforms_device((B, G), I.seed_of("bench", "ua"), dev)
+    v_us = I.uniforms_device((B,), I.seed_of("bench", "us"), dev)
+    v_acc = torch.empty((B,), dtype=torch.int32, device=dev)
+    v_out = torch.empty((B, G + 1), dtype=torch.int32, device=dev)
+    torch.cuda.synchronize()
+
+    launches_per_step = len(linears) + len(Ms) * len(linears) + 1
+
+    def step_body(c, mark):
+        mark()
+        for n, N, K in linears:
+            er.quantize_pack(src[c][n], qw[c][n], sc[c][n])
+        mark()
+        for i, M in enumerate(Ms):
+            cc = (c + 1 + i) % L
+            for n, N, K in linears:
+                er.w4a16_gemm(X[(M, K)], qw[cc][n], sc[cc][n], y=Y[n][:M], workspace=ws)
+                mark()
+        er.spec_verify(v_tgt, v_drf, v_tok, v_ua, v_us, True, 1.0, v_acc, v_out)
+        mark()
+
+    step_body(0, lambda: None)      # eager once: one-time function attributes / driver entry points, before capture
+    torch.cuda.synchronize()
+
+    # ---- capture one graph per rotation phase, external timing events around every launch -----------
+    mode = args.mode
+    graphs, events = [], []
+    if mode == "graph":
+        try:
+            side = torch.cuda.Stream()
+            for c in range(L):
+                evs = []
+
+                def mark():
+                    e = torch.cuda.Event(enable_timing=True, external=True)
+                    e.record()
+                    evs.append(e)
+                g = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(g, stream=side):
+                    step_body(c, mark)
+                graphs.append(g)
+                events.append(evs)
+        except Exception as e:
+            log(f"[bench] graph capture failed ({type(e).__name__}: {e}); falling back to stream launches")
+            mode, graphs, events = "stream", [], []
+            torch.cuda.synchronize()
+    if mode == "stream":
+        events = [[] for _ in range(L)]
+
+    def run_step(s):
+        c = s % L
+        if mode == "graph":
+            graphs[c].replay()
+        else:
+            evs = []
+
+            def mark():
+                e = torch.cuda.Event(enable_timing=True)
+                e.record()
+                evs.append(e)
+            step_body(c, mark)
+            events[c] = evs
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    for s in range(args.warmup):
+        run_step(s)
+    torch.cuda.synchronize()
+    barrier()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(local_rank)
+    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    sampler.start()
+    if mode == "stream":
+        torch.cuda._sleep(int(3e6))   # let the host run ahead of the device so launches queue back to back
+    t_start.record()
+    for s in range(args.steps):
+        run_step(args.warmup + s)
+    t_end.record()
+    torch.cuda.synchronize()
+    sampler.stop()
+    barrier()
+    step_ms = t_start.elapsed_time(t_end) / max(args.steps, 1)
+
+    # ---- per-launch durations from the events of the last replay of every phase that ran ------------
+    phases = [c for c in range(L) if any(((args.warmup + s) % L) == c for s in range(args.steps))] or [0]
+    nev = 2 + len(Ms) * len(linears) + 1
+    dur = torch.zeros((len(phases), nev - 1), dtype=torch.float64)
+    for pi, c in enumerate(phases):
+        evs = events[c]
+        assert len(evs) == nev
+        for i in range(nev - 1):
+            dur[pi, i] = evs[i].elapsed_time(evs[i + 1])
+    dur_ms = dur.mean(dim=0)                                   # [refresh, 36 gemm launches, verify]
+    stats = torch.cat([dur_ms, torch.tensor([step_ms], dtype=torch.float64)])
+    if dist is not None:                                        # max over ranks, on the device
+        t = stats.to(dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        stats = t.cpu()
+    dur_ms, step_ms = stats[:-1], float(stats[-1])
+
+    peak, peak_src = hbm_peak()
+    refresh_ms = float(dur_ms[0])
+    verify_ms = float(dur_ms[-1])
+    refresh_bytes = sum(REFRESH_BYTES_PER_ELEM * N * K for _, N, K in linears)
+    gemm_table, small_bytes, small_ms = [], 0.0, 0.0
+    k16_bytes, k16_ms, k16_n = 0.0, 0.0, 0
+    for i, M in enumerate(Ms):
+        row = {"M": M, "per_linear": {}}
+        tb, tm = 0.0, 0.0
+        for j, (n, N, K) in enumerate(linears):
+            ms = float(dur_ms[1 + i * len(linears) + j])
+            by = gemm_bytes(M, N, K)
+            tb, tm = tb + by, tm + ms
+            row["per_linear"][n] = {"us": round(ms * 1e3, 2), "gbs": round(by / ms / 1e6, 1),
+                                    "tflops": round(2.0 * M * N * K / ms / 1e9, 1)}
+            if M <= 16:
+                k16_bytes, k16_ms, k16_n = k16_bytes + by, k16_ms + ms, k16_n + 1
+        row.update({"layer_us": round(tm * 1e3, 2), "gbs": round(tb / tm / 1e6, 1),
+                    "frac_of_measured_peak": round(tb / tm / 1e6 / peak, 4),
+                    "frac_of_nominal_8tbs": round(tb / tm / 1e6 / NOMINAL_HBM_GBS, 4)})
+        gemm_table.append(row)
+        if M <= 16:
+            small_bytes, small_ms = small_bytes + tb, small_ms + tm
+    value = small_bytes * world / small_ms / 1e6               # GB/s, whole job
+    achieved = k16_bytes / k16_ms / 1e6
+    verify_bytes = B * (2 * G + 1) * V * 2.0
+
+    # ---- end-to-end leg: the same step through the *_host entry points ---------------------------------
+    e2e = None
+    if not args.no_e2e:
+        e2e = e2e_leg(args, er, I, torch, dev, linears, Ms, qw, sc, dist, world,
+                      (v_tgt, v_drf, v_tok, v_ua, v_us), small_bytes)
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu:
+        cpu = cpu_baseline_leg()
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": round(step_ms, 4), "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": "config1: 7B decoder-layer linear set (QKV 4608x3584, O 3584x3584, gate/up "
+                                   "37888x3584, down 3584x18944), W4A16 g128, M in {1..256}; step = refresh of the "
+                                   "layer + 36 GEMMs + config-4 verify (B=64, gamma=4, V=152064, bf16 logits)",
+                       "launch": mode, "l2": f"inputs larger than L2: {L} distinct layer copies (470 MB packed) "
+                                             "rotated per M; refresh streams 466 MB; verify 175 MB",
+                       "per_gpu": "every rank runs the same step on its own sequences/weights (replicas)"},
+            "clocks": sampler.summary(),
+            "e2e": e2e,
+            "gpu_launches": launches_per_step * args.steps,
+            "roofline": {"bound": "hbm", "kernel": "w4a16_gemm_kernel<16> (all M<=16 launches of the step)",
+                         "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+                         "frac": round(achieved / peak, 4), "traffic": NCU_TRAFFIC_BYTES, "peak_source": peak_src,
+                         "bytes_per_launch": round(k16_bytes / k16_n), "us_per_launch": round(k16_ms / k16_n * 1e3, 2)},
+            "cpu_baseline": cpu,
+            "detail": {
+                "gemm_vs_m": gemm_table,
+                "refresh": {"us": round(refresh_ms * 1e3, 1), "gbs": round(refresh_bytes / refresh_ms / 1e6, 1),
+                            "frac_of_measured_peak": round(refresh_bytes / refresh_ms / 1e6 / peak, 4),
+                            "elements": int(sum(N * K for _, N, K in linears))},
+                "verify": {"us": round(verify_ms * 1e3, 1), "B": B, "gamma": G, "V": V,
+                           "gbs_if_all_rows_read": round(verify_bytes / verify_ms / 1e6, 1),
+                           "mean_accept": round(float(v_acc.float().mean()), 3)},
+            },
+        }
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def e2e_leg(args, er, I, torch, dev, linears, Ms, qw, sc, dist, world, verify_dev, small_bytes):
+    """The same step with HOST buffers through er_*_host: per step the bf16 weights of the layer, every X and
+    the verify inputs are copied host->device from pinned memory and every Y and the verify outputs are read
+    back, inside the timed region."""
+    L = LAYER_COPIES
+    pin = lambda t: t.cpu().pin_memory()
+    w_host = {n: pin(I.weight_bf16(N, K, I.seed_of("bench", 0, n), device=dev)) for n, N, K in linears}
+    Ks = sorted({K for _, _, K in linears})
+    x_host = {(M, K): pin(I.activation_bf16(M, K, I.seed_of("bench", "x", M, K), device=dev)) for M in Ms for K in Ks}
+    y_host = {n: torch.empty((max(Ms), N), dtype=torch.bfloat16).pin_memory() for n, N, K in linears}
+    vt, vd, vx, vua, vus = [pin(t) for t in verify_dev]
+    B, G1, V = vt.shape
+    acc_h = torch.empty((B,), dtype=torch.int32).pin_memory()
+    out_h = torch.empty((B, G1), dtype=torch.int32).pin_memory()
+    lib = er.load()
+    need = max([lib.er_quantize_host_arena_bytes(N, K) for _, N, K in linears] +
+               [lib.er_gemm_host_arena_bytes(M, N, K) for M in Ms for _, N, K in linears] +
+               [lib.er_verify_host_arena_bytes(B, G1 - 1, V, er.ER_BF16)])
+    arena = er.host_arena(need, dev)
+    h2d = sum(t.numel() * t.element_size() for t in w_host.values())
+    h2d += sum(x_host[(M, K)].numel() * 2 for M in Ms for _, _, K in linears)
+    h2d += sum(t.numel() * t.element_size() for t in (vt, vd, vx, vua, vus))
+    d2h = sum(M * N * 2 for M in Ms for _, N, _ in linears) + acc_h.numel() * 4 + out_h.numel() * 4
+
+    def step(s, ev):
+        c = s % L
+        ev[0].record()
+        for n, N, K in linears:
+            er.quantize_pack_host(w_host[n], qw[c][n], sc[c][n], arena)
+        ev[1].record()
+        for i, M in enumerate(Ms):
+            if M == 32:
+                ev[2].record()
+            cc = (c + 1 + i) % L
+            for n, N, K in linears:
+                er.w4a16_gemm_host(x_host[(M, K)], qw[cc][n], sc[cc][n], y_host[n][:M], arena)
+        ev[3].record()
+        er.spec_verify_host(vt, vd, vx, vua, vus, True, 1.0, acc_h, out_h, arena)
+        ev[4].record()
+
+    steps = max(1, min(args.steps, 20))
+    mk = lambda: [torch.cuda.Event(enable_timing=True) for _ in range(5)]
+    for s in range(2):
+        step(s, mk())
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    evs = [mk() for _ in range(steps)]
+    for s in range(steps):
+        step(s, evs[s])
+    torch.cuda.synchronize()
+    seg = torch.zeros(4, dtype=torch.float64)
+    for ev in evs:
+        for i in range(4):
+            seg[i] += ev[i].elapsed_time(ev[i + 1]) / steps
+    if dist is not None:
+        t = seg.to(dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        seg = t.cpu()
+    refresh_ms, small_ms, large_ms, verify_ms = [float(v) for v in seg]
+    return {"value": round(small_bytes * world / small_ms / 1e6, 1), "unit": UNIT,
+            "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h), "steps": steps,
+            "ms_per_step": round(refresh_ms + small_ms + large_ms + verify_ms, 3),
+            "gemm_m_le_16_us": round(small_ms * 1e3, 1), "refresh_ms": round(refresh_ms, 3),
+            "verify_ms": round(verify_ms, 3),
+            "api": "er_quantize_pack_host / er_w4a16_gemm_host / er_spec_verify_host (pinned host buffers)"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=40)
+    ap.add_argument("--warmup", type=int, default=4)
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--mode", choices=["graph", "stream"], default="graph")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return reference_arm(args)
+    return product_arm(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -129,6 +129,33 @@ int er_spec_verify(const void* target, const void* draft, int in_dtype, int inpu
 /* Parity helper: qweight uint32 [N][K/8] -> int8 codes [N][K] in [-8, 7] (device). Not timed. */
 int er_unpack_codes(const void* qweight, int64_t N, int64_t K, int8_t* codes_out, void* stream);
 
+/* ---- HOST-buffer forms of the three calls (the end-to-end path) -------------------------------------
+ * Same operations and results as the device forms above.  Pointers named *_host are caller-owned HOST
+ * buffers (pinned memory makes the copies asynchronous; pageable memory works, staged by the runtime),
+ * dense (leading dimension = row length).  `arena` is a caller-owned DEVICE scratch buffer of at least
+ * er_*_host_arena_bytes(...) bytes, 16-byte aligned; each call stages its host operands into it
+ * (cudaMemcpyAsync on `stream`), runs the kernels, and copies results back to the host buffers, all on
+ * `stream` without synchronising: host outputs are valid once the stream reaches the end of the call, and
+ * host inputs must stay untouched until then.  Errors as above, plus ER_ERR_WORKSPACE for a small arena.
+ *   er_quantize_pack_host  W comes from the host; qweight_out / scales_out stay DEVICE pointers (they are
+ *                          the drafter's resident weights, consumed by er_w4a16_gemm).
+ *   er_w4a16_gemm_host     X from the host, Y to the host; qweight / scales are DEVICE pointers.  The first
+ *                          ER_GEMM_COUNTER_BYTES of ANY arena are reserved for the GEMM's tile counters (the
+ *                          other two calls never stage over them, so one arena serves all three): zero them
+ *                          once with er_gemm_workspace_init(arena, ...) before the first call.
+ *   er_spec_verify_host    every operand on the host. */
+size_t er_quantize_host_arena_bytes(int64_t N, int64_t K);
+size_t er_gemm_host_arena_bytes(int64_t M, int64_t N, int64_t K);
+size_t er_verify_host_arena_bytes(int32_t B, int32_t gamma, int32_t V, int in_dtype);
+int er_quantize_pack_host(const void* w_host, int64_t N, int64_t K, int group, void* qweight_out, void* scales_out,
+                          void* arena, size_t arena_bytes, void* stream);
+int er_w4a16_gemm_host(const void* x_host, int64_t M, int64_t K, const void* qweight, const void* scales, int64_t N,
+                       int group, void* y_host, int y_dtype, void* arena, size_t arena_bytes, void* stream);
+int er_spec_verify_host(const void* target_host, const void* draft_host, int in_dtype, int inputs_are_logits,
+                        float temperature, const int32_t* draft_tokens_host, const float* u_accept_host,
+                        const float* u_sample_host, int32_t B, int32_t gamma, int32_t V, int32_t* accept_count_host,
+                        int32_t* out_tokens_host, void* arena, size_t arena_bytes, void* stream);
+
 #ifdef __cplusplus
 }
 #endif

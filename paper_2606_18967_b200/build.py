@@ -11,7 +11,7 @@ PKG_DIR = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(PKG_DIR, "csrc")
 INCLUDE = os.path.join(os.path.dirname(PKG_DIR), "include")
 LIB_PATH = os.path.join(PKG_DIR, "liber_b200.so")
-SOURCES = ["er_api.cu", "quantize_pack.cu", "spec_verify.cu", "w4a16_gemm_simt.cu", "w4a16_gemm.cu"]
+SOURCES = ["er_api.cu", "er_host.cu", "quantize_pack.cu", "spec_verify.cu", "w4a16_gemm_simt.cu", "w4a16_gemm.cu"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC]
 

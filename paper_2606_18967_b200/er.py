@@ -61,6 +61,19 @@ def load() -> ctypes.CDLL:
     lib.er_spec_verify.argtypes = [vp, vp, ctypes.c_int, ctypes.c_int, f32, vp, vp, vp, i32, i32, i32, vp, vp, vp]
     lib.er_unpack_codes.restype = ctypes.c_int
     lib.er_unpack_codes.argtypes = [vp, i64, i64, vp, vp]
+    lib.er_quantize_host_arena_bytes.restype = sz
+    lib.er_quantize_host_arena_bytes.argtypes = [i64, i64]
+    lib.er_gemm_host_arena_bytes.restype = sz
+    lib.er_gemm_host_arena_bytes.argtypes = [i64, i64, i64]
+    lib.er_verify_host_arena_bytes.restype = sz
+    lib.er_verify_host_arena_bytes.argtypes = [i32, i32, i32, ctypes.c_int]
+    lib.er_quantize_pack_host.restype = ctypes.c_int
+    lib.er_quantize_pack_host.argtypes = [vp, i64, i64, ctypes.c_int, vp, vp, vp, sz, vp]
+    lib.er_w4a16_gemm_host.restype = ctypes.c_int
+    lib.er_w4a16_gemm_host.argtypes = [vp, i64, i64, vp, vp, i64, ctypes.c_int, vp, ctypes.c_int, vp, sz, vp]
+    lib.er_spec_verify_host.restype = ctypes.c_int
+    lib.er_spec_verify_host.argtypes = [vp, vp, ctypes.c_int, ctypes.c_int, f32, vp, vp, vp, i32, i32, i32, vp, vp, vp,
+                                        sz, vp]
     lib.er_gemm_tuning.restype = ctypes.c_int
     lib.er_gemm_tuning.argtypes = [ctypes.c_int, ctypes.c_int]
     if lib.er_abi_version() != 1:
@@ -170,3 +183,54 @@ def unpack_codes(qweight: torch.Tensor) -> torch.Tensor:
     codes = torch.empty((N, J * 8), dtype=torch.int8, device=qweight.device)
     _check(load().er_unpack_codes(qweight.data_ptr(), N, J * 8, codes.data_ptr(), _stream(qweight)), "er_unpack_codes")
     return codes
+
+
+# ---- host-buffer forms (include/er.h "HOST-buffer forms"): host tensors in / out, device arena for staging ----
+
+def _host(t: torch.Tensor, name: str):
+    if t.is_cuda or not t.is_contiguous():
+        raise ValueError(f"{name} must be a contiguous host tensor")
+
+
+def host_arena(nbytes: int, device) -> torch.Tensor:
+    """Device staging arena for the *_host calls; GEMM tile counters (its first bytes) zeroed."""
+    arena = torch.empty(max(int(nbytes), COUNTER_BYTES), dtype=torch.uint8, device=device)
+    _check(load().er_gemm_workspace_init(arena.data_ptr(), arena.numel(), _stream(arena)), "er_gemm_workspace_init")
+    return arena
+
+
+def quantize_pack_host(w_host: torch.Tensor, qweight: torch.Tensor, scales: torch.Tensor, arena: torch.Tensor):
+    _host(w_host, "w_host")
+    N, K = w_host.shape
+    _check(load().er_quantize_pack_host(w_host.data_ptr(), N, K, GROUP, qweight.data_ptr(), scales.data_ptr(),
+                                        arena.data_ptr(), arena.numel(), _stream(arena)), "er_quantize_pack_host")
+    return qweight, scales
+
+
+def w4a16_gemm_host(x_host: torch.Tensor, qweight: torch.Tensor, scales: torch.Tensor, y_host: torch.Tensor,
+                    arena: torch.Tensor):
+    _host(x_host, "x_host")
+    _host(y_host, "y_host")
+    M, K = x_host.shape
+    N = qweight.shape[0]
+    ydt = ER_F32 if y_host.dtype == torch.float32 else ER_BF16
+    _check(load().er_w4a16_gemm_host(x_host.data_ptr(), M, K, qweight.data_ptr(), scales.data_ptr(), N, GROUP,
+                                     y_host.data_ptr(), ydt, arena.data_ptr(), arena.numel(), _stream(arena)),
+           "er_w4a16_gemm_host")
+    return y_host
+
+
+def spec_verify_host(target: torch.Tensor, draft: torch.Tensor, draft_tokens: torch.Tensor, u_accept: torch.Tensor,
+                     u_sample: torch.Tensor, inputs_are_logits: bool, temperature: float,
+                     accept_count: torch.Tensor, out_tokens: torch.Tensor, arena: torch.Tensor):
+    for t, n in ((target, "target"), (draft, "draft"), (draft_tokens, "draft_tokens"), (u_accept, "u_accept"),
+                 (u_sample, "u_sample"), (accept_count, "accept_count"), (out_tokens, "out_tokens")):
+        _host(t, n)
+    B, G1, V = target.shape
+    dt = ER_F32 if target.dtype == torch.float32 else ER_BF16
+    _check(load().er_spec_verify_host(target.data_ptr(), draft.data_ptr(), dt, int(inputs_are_logits),
+                                      float(temperature), draft_tokens.data_ptr(), u_accept.data_ptr(),
+                                      u_sample.data_ptr(), B, G1 - 1, V, accept_count.data_ptr(),
+                                      out_tokens.data_ptr(), arena.data_ptr(), arena.numel(), _stream(arena)),
+           "er_spec_verify_host")
+    return accept_count, out_tokens

@@ -130,3 +130,30 @@ def sample_draft_tokens(q_probs: np.ndarray, seed) -> np.ndarray:
             r = rng.random() * c[-1]
             out[b, i] = min(int(np.searchsorted(c, r, side="right")), V - 1)
     return out
+
+
+# ---- device-side generators for the full-size workloads (bench.py; too large for the numpy path) -----
+
+def verify_logits_bf16_device(B, gamma, V, seed, device, std=2.0, draft_noise=0.5):
+    """Config-4 verify inputs generated on `device`: target bf16 [B, gamma+1, V] = bf16(N(0, std^2)),
+    draft bf16 [B, gamma, V] = bf16(target_fp32 + N(0, draft_noise^2)) on the first gamma positions."""
+    g = _gen(device, seed)
+    tgt32 = torch.empty((B, gamma + 1, V), dtype=torch.float32, device=device).normal_(0.0, std, generator=g)
+    noise = torch.empty((B, gamma, V), dtype=torch.float32, device=device).normal_(0.0, draft_noise, generator=g)
+    drf = (tgt32[:, :gamma, :] + noise).to(torch.bfloat16)
+    return tgt32.to(torch.bfloat16), drf
+
+
+def sample_draft_tokens_gumbel(draft_logits: torch.Tensor, seed, temperature=1.0) -> torch.Tensor:
+    """x_i ~ softmax(draft_logits_i / T) by the Gumbel-max trick (argmax of logit/T + Gumbel noise): an exact
+    sampler that needs no normalisation, so no part of the method's arithmetic lives here.  int32 [B, gamma]."""
+    g = _gen(draft_logits.device, seed)
+    u = torch.empty(draft_logits.shape, dtype=torch.float32, device=draft_logits.device).uniform_(1e-20, 1.0, generator=g)
+    gumbel = -torch.log(-torch.log(u))
+    return torch.argmax(draft_logits.float() / temperature + gumbel, dim=-1).to(torch.int32)
+
+
+def uniforms_device(shape, seed, device):
+    """fp32 uniforms in [0, 1) on `device`."""
+    g = _gen(device, seed)
+    return torch.empty(shape, dtype=torch.float32, device=device).uniform_(0.0, 1.0, generator=g).clamp_(max=1.0 - 2.0 ** -24)
