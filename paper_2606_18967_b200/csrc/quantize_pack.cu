@@ -1,11 +1,21 @@
 // quantize_pack.cu -- er_quantize_pack: the per-RL-step drafter refresh ("lightweight RTN
 // quantization to the FFN and QKVO projection layers", L150 Alg. 1 line 3) and er_unpack_codes.
 //
-// HBM-bound streaming kernel: 2 B read + 0.5 B + 2/128 B written per element.
-// One CTA quantizes a tile of 32 rows x 512 k.  A lane owns 8 consecutive k (one 128-bit load, one 32-bit
-// packed word out); 16 lanes cover one 128-element group, so the group max is 4 shuffle-xor steps.  All 8
-// loads of a thread are issued before any arithmetic (128 B in flight per thread).  The 4 x 32 scales of
-// the tile are transposed through shared memory so that they leave as 64-byte runs along N.
+// HBM-bound streaming kernel: 2 B read + 0.5 B + 2/128 B written per element.  The first
+// version was instruction-bound (ncu: issue 75 %, DRAM 35 %), so the arithmetic is cut to ~7 instructions per
+// element:
+//   - a lane owns 16 consecutive k (ONE 256-bit load, two packed words out); 8 lanes cover a 128-element group,
+//     so the group max is 3 shuffle-xor steps, taken on packed bf16x2 |w| (half the compares);
+//   - scale s = bf16_rne(amax * (1/7)): identical to the IEEE division for every bf16 amax (Q4: a/7 is
+//     never within 2^-12 relative of a bf16 rounding boundary);
+//   - q = rint(w / s) with IEEE-division semantics AT TIES (Q6): t = w * r with r ~ 1/s (MUFU.RCP),
+//     one exact-residual Newton step (returns k + 1/2 exactly whenever w / s is exactly k + 1/2; every non-tie
+//     quotient of two 8-bit significands is >= 1/1020 from a tie, far above the 1e-6 error of t);
+//   - rounding + offset in one FADD: bits(t + (1.5 * 2^23 + 8)) = 0x4B400000 + (q + 8), RNE on the integer grid;
+//   - nibble placement by integer multiply-add of those bits (the constant upper bits are removed once per word).
+// A CTA quantizes a tile of 32 rows x 512 k; a warp takes 4 rows, all 4 loads issued before any arithmetic.  The
+// 4 x 32 scales of the tile are transposed through shared memory so that they leave as 64-byte runs along N.
+#include <cuda_bf16.h>
 #include "er_common.cuh"
 
 namespace {
@@ -13,9 +23,19 @@ namespace {
 constexpr int kTileRows = 32;
 constexpr int kTileK = 512;
 constexpr int kThreads = 256;
-constexpr int kIters = 8;  // (row, 256-wide half) pairs per warp: 4 rows x 2 halves
+constexpr int kIters = 4;  // rows per warp
 
-__device__ __forceinline__ uint4 ld_stream(const uint4* p) {
+struct U8 { uint32_t v[8]; };
+
+__device__ __forceinline__ U8 ld_stream256(const void* p) {
+  U8 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v8.u32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r.v[0]), "=r"(r.v[1]), "=r"(r.v[2]), "=r"(r.v[3]), "=r"(r.v[4]), "=r"(r.v[5]), "=r"(r.v[6]),
+                 "=r"(r.v[7])
+               : "l"(p));
+  return r;
+}
+__device__ __forceinline__ uint4 ld_stream128(const void* p) {
   uint4 r;
   asm volatile("ld.global.nc.L1::no_allocate.v4.u32 {%0, %1, %2, %3}, [%4];"
                : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w)
@@ -23,86 +43,115 @@ __device__ __forceinline__ uint4 ld_stream(const uint4* p) {
   return r;
 }
 
-// q = clamp(rint(w / s), -8, 7) + 8 with IEEE-division semantics at the ties that matter (Q6):
-// t = w * r (r = rn(1/s)) is refined by one exact-residual Newton step, which returns k + 1/2 exactly
-// whenever w / s is exactly k + 1/2, and is otherwise within ~1e-6 of w / s while every non-tie quotient
-// of two 8-bit significands is >= 1/1020 away from a tie.
-__device__ __forceinline__ uint32_t code_of(float w, float s, float r) {
-  float t = w * r;
-  float e = __fmaf_rn(-t, s, w);
-  t = __fmaf_rn(e, r, t);
-  float q = rintf(t);
-  q = fminf(fmaxf(q, -8.0f), 7.0f);
-  return (uint32_t)(__float2int_rn(q) + 8);
+// packed bf16x2 max(|a|, |b|) in ONE instruction; the result's sign bits are xor-of-signs garbage, which the
+// next absmax2 (or the final mask) discards.
+__device__ __forceinline__ uint32_t absmax2(uint32_t a, uint32_t b) {
+  uint32_t d;
+  asm("max.xorsign.abs.bf16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
+  return d;
 }
-__device__ __forceinline__ uint32_t code_of_div(float w, float s) {
-  float q = rintf(__fdiv_rn(w, s));
-  q = fminf(fmaxf(q, -8.0f), 7.0f);
-  return (uint32_t)(__float2int_rn(q) + 8);
+
+constexpr float kMagic = 12582912.0f + 8.0f;  // 1.5 * 2^23 + 8: bits(t + kMagic) = 0x4B400000 + rint(t) + 8
+
+// bits whose low nibble is the stored code u = rint(w / s) + 8 (upper 28 bits = 0x4B40000)
+__device__ __forceinline__ uint32_t code_bits(float w, float s, float r) {
+  float t = w * r;
+  const float e = __fmaf_rn(-t, s, w);
+  t = __fmaf_rn(e, r, t);
+  return __float_as_uint(t + kMagic);
+}
+__device__ __forceinline__ uint32_t code_bits_div(float w, float s) {  // denormal scales: plain IEEE division
+  return __float_as_uint(__fdiv_rn(w, s) + kMagic);
+}
+
+// Packs the 8 codes of 4 raw words (k = 0..7 of the word) into one ER_PACK_V1 word: logical k = 2 t + h sits in
+// nibble t + 4 h.  `sum of (0x4B400000 << 4 i)` over i = 0..7 (mod 2^32) is the constant removed at the end.
+template <bool kDiv>
+__device__ __forceinline__ uint32_t pack8(const uint32_t* raw, float s, float r) {
+  uint32_t acc = 0;
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    const float lo = __uint_as_float(raw[t] << 16);
+    const float hi = __uint_as_float(raw[t] & 0xFFFF0000u);
+    const uint32_t bl = kDiv ? code_bits_div(lo, s) : code_bits(lo, s, r);
+    const uint32_t bh = kDiv ? code_bits_div(hi, s) : code_bits(hi, s, r);
+    acc += bl << (4 * t);
+    acc += bh << (4 * t + 16);
+  }
+  constexpr uint32_t kConst = 0x4B400000u * 0x11111111u;  // sum_i 0x4B400000 << 4 i  (mod 2^32)
+  return acc - kConst;
+}
+
+// cold path (denormal scale: 1/s would overflow), kept out of line; reloads its 16 elements so that the hot
+// path's registers never need an address
+__device__ __noinline__ uint2 pack16_div(const uint16_t* src, float s) {
+  const uint4 a = *reinterpret_cast<const uint4*>(src), b = *reinterpret_cast<const uint4*>(src + 8);
+  const uint32_t r0[4] = {a.x, a.y, a.z, a.w}, r1[4] = {b.x, b.y, b.z, b.w};
+  return make_uint2(pack8<true>(r0, s, 0.f), pack8<true>(r1, s, 0.f));
 }
 
 __global__ void __launch_bounds__(kThreads) quantize_pack_kernel(const uint16_t* __restrict__ w, int64_t N,
                                                                  int64_t K, int64_t ldw,
                                                                  uint32_t* __restrict__ qweight,
-                                                                 uint16_t* __restrict__ scales) {
+                                                                 uint16_t* __restrict__ scales, int vec256) {
   __shared__ uint16_t s_scales[kTileK / ER_GROUP][kTileRows];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t n0 = (int64_t)blockIdx.y * kTileRows;
-  const int64_t k0 = (int64_t)blockIdx.x * kTileK;
+  const int64_t k = (int64_t)blockIdx.x * kTileK + lane * 16;
 
-  uint4 v[kIters];
+  U8 v[kIters];
   bool ok[kIters];
 #pragma unroll
   for (int it = 0; it < kIters; ++it) {
-    const int r = warp * 4 + (it >> 1);
-    const int64_t n = n0 + r;
-    const int64_t k = k0 + (it & 1) * 256 + lane * 8;
+    const int64_t n = n0 + warp * kIters + it;
     ok[it] = (n < N) && (k < K);
-    v[it] = make_uint4(0, 0, 0, 0);
-    if (ok[it]) v[it] = ld_stream(reinterpret_cast<const uint4*>(w + n * ldw + k));
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[it].v[i] = 0;
+    if (ok[it]) {
+      const uint16_t* src = w + n * ldw + k;
+      if (vec256) {
+        v[it] = ld_stream256(src);
+      } else {  // rows only 16-byte aligned
+        const uint4 a = ld_stream128(src), b = ld_stream128(src + 8);
+        v[it].v[0] = a.x; v[it].v[1] = a.y; v[it].v[2] = a.z; v[it].v[3] = a.w;
+        v[it].v[4] = b.x; v[it].v[5] = b.y; v[it].v[6] = b.z; v[it].v[7] = b.w;
+      }
+    }
   }
 
 #pragma unroll
   for (int it = 0; it < kIters; ++it) {
-    const int r = warp * 4 + (it >> 1);
-    const uint32_t raw[4] = {v[it].x, v[it].y, v[it].z, v[it].w};
-    float f[8];
+    const int r_in_tile = warp * kIters + it;
+    const uint32_t* raw = v[it].v;
+    uint32_t m2 = absmax2(absmax2(absmax2(raw[0], raw[1]), absmax2(raw[2], raw[3])),
+                          absmax2(absmax2(raw[4], raw[5]), absmax2(raw[6], raw[7])));
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      f[2 * i] = __uint_as_float(raw[i] << 16);
-      f[2 * i + 1] = __uint_as_float(raw[i] & 0xFFFF0000u);
-    }
-    float amax = 0.0f;
-#pragma unroll
-    for (int i = 0; i < 8; ++i) amax = fmaxf(amax, fabsf(f[i]));
-#pragma unroll
-    for (int off = 1; off < 16; off <<= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, off));
-
-    const __nv_bfloat16 sb = __float2bfloat16_rn(__fdiv_rn(amax, 7.0f));
+    for (int off = 1; off < 8; off <<= 1) m2 = absmax2(m2, __shfl_xor_sync(0xffffffffu, m2, off));
+    const float amax = fmaxf(fabsf(__uint_as_float(m2 << 16)), fabsf(__uint_as_float(m2 & 0xFFFF0000u)));
+    const __nv_bfloat16 sb = __float2bfloat16_rn(amax * 0.142857149f);
     const float s = __bfloat162float(sb);
-    uint32_t word = 0x88888888u;  // all q = 0 (s == 0, Q8)
-    if (s > 0.0f) {
-      word = 0;
-      if (s >= 1e-30f) {
-        const float rcp = __frcp_rn(s);
-#pragma unroll
-        for (int i = 0; i < 8; ++i) word |= code_of(f[i], s, rcp) << (4 * ((i >> 1) + 4 * (i & 1)));
-      } else {  // 1/s would overflow: plain IEEE division
-#pragma unroll
-        for (int i = 0; i < 8; ++i) word |= code_of_div(f[i], s) << (4 * ((i >> 1) + 4 * (i & 1)));
-      }
+    uint32_t w0, w1;
+    if (s >= 1e-30f) {
+      float r;
+      asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(s));
+      w0 = pack8<false>(raw, s, r);
+      w1 = pack8<false>(raw + 4, s, r);
+    } else if (s > 0.0f) {
+      const uint2 pd = pack16_div(w + (n0 + r_in_tile) * ldw + k, s);
+      w0 = pd.x; w1 = pd.y;
+    } else {
+      w0 = w1 = 0x88888888u;  // all q = 0 (s == 0, Q8)
     }
     if (ok[it]) {
-      const int64_t n = n0 + r;
-      const int64_t k = k0 + (it & 1) * 256 + lane * 8;
-      qweight[n * (K >> 3) + (k >> 3)] = word;
+      const int64_t n = n0 + r_in_tile;
+      *reinterpret_cast<uint2*>(qweight + n * (K >> 3) + (k >> 3)) = make_uint2(w0, w1);
     }
-    if ((lane & 15) == 0) s_scales[(it & 1) * 2 + (lane >> 4)][r] = (s > 0.0f) ? __bfloat16_as_ushort(sb) : 0;
+    if ((lane & 7) == 0) s_scales[lane >> 3][r_in_tile] = (s > 0.0f) ? __bfloat16_as_ushort(sb) : 0;
   }
   __syncthreads();
   if (threadIdx.x < (kTileK / ER_GROUP) * kTileRows) {
     const int g = threadIdx.x >> 5, r = threadIdx.x & 31;
-    const int64_t gg = (k0 >> 7) + g, n = n0 + r;
+    const int64_t gg = ((int64_t)blockIdx.x * kTileK >> 7) + g, n = n0 + r;
     if (n < N && gg < (K >> 7)) scales[gg * N + n] = s_scales[g][r];
   }
 }
@@ -139,9 +188,10 @@ int er_quantize_pack(const void* w_bf16, int64_t N, int64_t K, int64_t ldw_elems
   // grid.x = k tiles (fastest) so that consecutive CTAs stream consecutive bytes of the same rows
   dim3 grid((unsigned)((K + kTileK - 1) / kTileK), (unsigned)((N + kTileRows - 1) / kTileRows));
   if (grid.y > 65535u) return ER_ERR_SHAPE;  // N > 2,097,120 rows: split the call
+  const int vec256 = ((reinterpret_cast<uintptr_t>(w_bf16) & 31u) == 0 && (ldw_elems % 16) == 0) ? 1 : 0;
   quantize_pack_kernel<<<grid, kThreads, 0, (cudaStream_t)stream>>>(
       reinterpret_cast<const uint16_t*>(w_bf16), N, K, ldw_elems, reinterpret_cast<uint32_t*>(qweight_out),
-      reinterpret_cast<uint16_t*>(scales_out));
+      reinterpret_cast<uint16_t*>(scales_out), vec256);
   ER_CUDA_TRY(cudaGetLastError());
   return ER_OK;
 }
