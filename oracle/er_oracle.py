@@ -87,29 +87,57 @@ def quantize_codes(w_u16: np.ndarray, group: int = GROUP):
     return codes, np.ascontiguousarray(s_u16.T)                        # scales [G][N]
 
 
+TILE_ROWS = 128      # rows of W per packed block (Q11, ER_PACK_V2)
+
+
+def _word_slot(r: np.ndarray, j: np.ndarray) -> np.ndarray:
+    """ER_PACK_V2 (Q11): position, in 32-bit words, of logical word j (0..15, 8 codes each) of row r
+    (0..127) inside its 128-row x 128-k block of 128 x 16 words: the row keeps its place, its four 16-byte chunks
+    are permuted by XOR with bits 1..2 of the row index."""
+    chunk, within = j // 4, j % 4
+    return r * 16 + (chunk ^ ((r >> 1) & 3)) * 4 + within
+
+
 def pack_codes(codes: np.ndarray) -> np.ndarray:
-    """int8 codes [N][K] in [-8,7] -> uint32 qweight [N][K/8] (ER_PACK_V1, DESIGN.md
-    Q10-Q11): stored nibble u = q + 8 (offset binary); word (n, j) carries logical
-    k = 8 j + PACK_PERM[i] in bits [4 i, 4 i + 4)."""
+    """int8 codes [N][K] in [-8,7] -> uint32 qweight, N*K/8 words returned as [N][K/8] (ER_PACK_V2, DESIGN.md
+    Q10-Q11).  Stored nibble u = q + 8 (offset binary); a word carries the 8 codes of logical k = 8 j + PACK_PERM[i]
+    in bits [4 i, 4 i + 4).  Words are stored block by block: block (T, g) = rows 128 T .. 128 T + 127, k = 128 g ..
+    128 g + 127, blocks ordered T-major then g, each block 128 x 16 words laid out by _word_slot."""
     codes = np.asarray(codes, dtype=np.int8)
     N, K = codes.shape
-    assert K % 8 == 0
+    assert K % GROUP == 0 and N % TILE_ROWS == 0
     u = (codes.astype(np.int32) + 8).astype(np.uint32).reshape(N, K // 8, 8)
-    word = np.zeros((N, K // 8), dtype=np.uint32)
+    word = np.zeros((N, K // 8), dtype=np.uint32)          # word[n][jj], jj = k // 8 (row-major, logical)
     for i in range(8):
         word |= u[:, :, PACK_PERM[i]] << np.uint32(4 * i)
-    return word
+    T, G = N // TILE_ROWS, K // GROUP
+    out = np.zeros((T, G, TILE_ROWS * 16), dtype=np.uint32)
+    r = np.arange(TILE_ROWS)[:, None]
+    j = np.arange(16)[None, :]
+    slot = _word_slot(r, j)                                 # [128][16]
+    blocks = word.reshape(T, TILE_ROWS, G, 16).transpose(0, 2, 1, 3)   # [T][G][r][j]
+    out[:, :, slot.reshape(-1)] = blocks.reshape(T, G, TILE_ROWS * 16)
+    return out.reshape(N, K // 8)
 
 
 def unpack_codes(qweight: np.ndarray) -> np.ndarray:
-    """Inverse of pack_codes: uint32 [N][K/8] -> int8 [N][K]."""
+    """Inverse of pack_codes: uint32 [N][K/8] (ER_PACK_V2 storage) -> int8 codes [N][K]."""
     qweight = np.asarray(qweight, dtype=np.uint32)
     N, J = qweight.shape
+    K = J * 8
+    assert K % GROUP == 0 and N % TILE_ROWS == 0
+    T, G = N // TILE_ROWS, K // GROUP
+    r = np.arange(TILE_ROWS)[:, None]
+    j = np.arange(16)[None, :]
+    slot = _word_slot(r, j)
+    stored = qweight.reshape(T, G, TILE_ROWS * 16)
+    blocks = stored[:, :, slot.reshape(-1)].reshape(T, G, TILE_ROWS, 16)
+    word = blocks.transpose(0, 2, 1, 3).reshape(N, J)       # logical word[n][k // 8]
     codes = np.empty((N, J, 8), dtype=np.int8)
     for i in range(8):
-        nib = (qweight >> np.uint32(4 * i)) & np.uint32(0xF)
+        nib = (word >> np.uint32(4 * i)) & np.uint32(0xF)
         codes[:, :, PACK_PERM[i]] = nib.astype(np.int32) - 8
-    return codes.reshape(N, J * 8)
+    return codes.reshape(N, K)
 
 
 def quantize_pack(w_u16: np.ndarray, group: int = GROUP):

@@ -19,7 +19,7 @@ def _bf16_fraction(u):
 
 def test_one_hot_reads_out_dequantized_matrix():
     # x[m] = e_k  ->  y[m][n] = q[n][k] * s[k//128][n] exactly
-    N, K = 16, 256
+    N, K = 128, 256
     codes = I.random_codes(N, K, seed=2)
     qw = O.pack_codes(codes)
     rng = np.random.default_rng(0)
@@ -34,7 +34,7 @@ def test_one_hot_reads_out_dequantized_matrix():
 
 def test_integer_probe_is_exact():
     # s = 1, X in {-1,0,1,2}, raw codes in [-8,7]: the result is an exact integer
-    N, K, M = 24, 1024, 5
+    N, K, M = 128, 1024, 5
     codes = I.random_codes(N, K, seed=4)
     rng = np.random.default_rng(7)
     xi = rng.integers(-1, 3, size=(M, K))
@@ -46,7 +46,7 @@ def test_integer_probe_is_exact():
 
 def test_against_exact_rational_brute_force():
     # tiny shape, pure-Python Fractions: transposed operands, wrong group index or dropped scale all fail here
-    N, K, M = 3, 256, 2
+    N, K, M = 128, 256, 2
     w = I.as_u16(I.weight_bf16(N, K, seed=11))
     x = I.as_u16(I.activation_bf16(M, K, seed=12))
     qw, scales = O.quantize_pack(w)
@@ -61,14 +61,15 @@ def test_against_exact_rational_brute_force():
 
 
 def test_k_split_invariance_and_linearity():
-    N, K, M = 32, 1024, 4
+    N, K, M = 128, 1024, 4
     w = I.as_u16(I.weight_bf16(N, K, seed=21))
     x = I.as_u16(I.activation_bf16(M, K, seed=22))
     qw, scales = O.quantize_pack(w)
     y = O.w4a16_gemm(x, qw, scales)
     acc = np.zeros_like(y)
     for g in range(K // 128):
-        acc += O.w4a16_gemm(x[:, g * 128:(g + 1) * 128], qw[:, g * 16:(g + 1) * 16], scales[g:g + 1])
+        qw_g = O.pack_codes(O.unpack_codes(qw)[:, g * 128:(g + 1) * 128])      # the packed form of one k-group
+        acc += O.w4a16_gemm(x[:, g * 128:(g + 1) * 128], qw_g, scales[g:g + 1])
     assert np.allclose(acc, y, rtol=1e-12, atol=1e-14)
     # linearity with bf16-exact operands: X and 2X
     x2 = O.f32_to_bf16_rne(O.bf16_to_f32(x) * np.float32(2))
@@ -77,7 +78,7 @@ def test_k_split_invariance_and_linearity():
 
 def test_quantized_matmul_close_to_unquantized():
     # the dequantized weight approximates W: relative Frobenius error of RTN-4bit g128 on N(0, .02) is ~ 9 %
-    N, K = 64, 1024
+    N, K = 128, 1024
     w = I.as_u16(I.weight_bf16(N, K, seed=31))
     qw, scales = O.quantize_pack(w)
     wd = O.dequantize(qw, scales)

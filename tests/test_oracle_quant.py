@@ -41,31 +41,41 @@ def test_bf16_helpers_roundtrip_all_patterns():
 
 
 def test_pack_roundtrip_every_nibble_every_position():
-    # all 16 nibble values at all 8 word positions (Q10)
-    codes = np.zeros((16, 8 * 8), dtype=np.int8)
+    # all 16 nibble values at all 8 word positions (Q10), in every 16-byte chunk of a block row
+    codes = np.zeros((128, 128), dtype=np.int8)
     for v in range(16):
         for pos in range(8):
-            codes[v, pos * 8 + pos] = v - 8
+            for chunk in range(4):
+                codes[8 * v + pos, 32 * chunk + pos * 4 % 32 + pos % 4] = v - 8
     packed = O.pack_codes(codes)
-    assert packed.dtype == np.uint32 and packed.shape == (16, 8)
+    assert packed.dtype == np.uint32 and packed.shape == (128, 16)
     assert np.array_equal(O.unpack_codes(packed), codes)
-    cc = I.counting_codes(64, 256)
+    rng = np.random.default_rng(1)
+    rc = rng.integers(-8, 8, size=(256, 384), dtype=np.int8)
+    assert np.array_equal(O.unpack_codes(O.pack_codes(rc)), rc)
+    cc = I.counting_codes(128, 256)
     assert np.array_equal(O.unpack_codes(O.pack_codes(cc)), cc)
 
 
 def test_pack_layout_is_the_documented_index_function():
-    # word (n, j) holds logical k = 8 j + pi[i] in bits [4i, 4i+4), pi = (0,2,4,6,1,3,5,7), nibble = q + 8 (Q11),
-    # written independently of the oracle's loop: (word >> 4t) & 0x000F000F yields the pair (k=2t, 2t+1).
+    # ER_PACK_V2 (Q11), written independently of the oracle's vectorised packer, element by element:
+    # block (T, g) of 128 rows x 128 k starts at word (T * G + g) * 2048; inside it row r keeps its place (16 words),
+    # its 16-byte chunks are XOR-permuted by (r >> 1) & 3; the word of logical k-octet j holds k = 8 j + pi[i] in
+    # bits [4i, 4i+4), pi = (0,2,4,6,1,3,5,7), nibble = q + 8: (word >> 4t) & 0x000F000F is the pair (k=2t, 2t+1).
     rng = np.random.default_rng(3)
-    codes = rng.integers(-8, 8, size=(5, 32), dtype=np.int8)
-    packed = O.pack_codes(codes)
-    for n in range(5):
-        for j in range(4):
-            wv = int(packed[n, j])
+    N, K = 256, 384
+    G = K // 128
+    codes = rng.integers(-8, 8, size=(N, K), dtype=np.int8)
+    flat = O.pack_codes(codes).reshape(-1)
+    for n in (0, 1, 2, 3, 5, 6, 127, 128, 131, 255):
+        for jj in range(K // 8):
+            T, r, g, j = n // 128, n % 128, jj // 16, jj % 16
+            idx = (T * G + g) * 2048 + r * 16 + ((j // 4) ^ ((r >> 1) & 3)) * 4 + j % 4
+            wv = int(flat[idx])
             for t in range(4):
                 pair = (wv >> (4 * t)) & 0x000F000F
-                assert (pair & 0xFFFF) - 8 == codes[n, 8 * j + 2 * t]
-                assert (pair >> 16) - 8 == codes[n, 8 * j + 2 * t + 1]
+                assert (pair & 0xFFFF) - 8 == codes[n, 8 * jj + 2 * t]
+                assert (pair >> 16) - 8 == codes[n, 8 * jj + 2 * t + 1]
 
 
 def test_error_bound_and_code_range_on_config_like_weights():
