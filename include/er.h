@@ -26,9 +26,13 @@
  *
  * Data layouts:
  *   W        bf16 [N][K], row-major, K contiguous, row stride ldw elements (torch nn.Linear.weight)
- *   qweight  uint32 [N][K/8] row-major ("ER_PACK_V1"): word (n, j) holds the 8 codes of logical
- *            k = 8 j + pi[i] in bits [4 i, 4 i + 4), pi = (0,2,4,6,1,3,5,7); stored nibble u = q + 8,
- *            q in [-8, 7].  So (word >> 4 t) & 0x000F000F is the pair (k = 8 j + 2 t, 8 j + 2 t + 1).
+ *   qweight  N*K/8 uint32 words, "ER_PACK_V2": blocks of 128 rows x 128 k (2048 words = 8 KiB, contiguous),
+ *            stored tile-major then group: block (T, g) starts at word (T * K/128 + g) * 2048.  Inside a block
+ *            row r keeps its place (16 words) and its four 16-byte chunks are XOR-permuted by (r >> 1) & 3: the
+ *            word of k-octet j (0..15) of row r sits at  r*16 + ((j/4) ^ ((r>>1)&3))*4 + j%4.  A word holds the
+ *            8 codes of logical k = 8 j + pi[i] in bits [4 i, 4 i + 4), pi = (0,2,4,6,1,3,5,7); stored nibble
+ *            u = q + 8, q in [-8, 7]: (word >> 4 t) & 0x000F000F is the pair (k = 8 j + 2 t, 8 j + 2 t + 1).
+ *            (One block = one contiguous, bank-conflict-free shared-memory stage of the GEMM.)
  *   scales   bf16 [K/128][N] (group-major, N contiguous); s = bf16_rne(max|w| / 7) per 128 consecutive k
  *   X        bf16 [M][K], row stride ldx elements
  *   Y        bf16 or fp32 [M][N], row stride ldy elements
@@ -78,8 +82,8 @@ int er_gemm_workspace_init(void* workspace, size_t workspace_bytes, void* stream
 
 /* (2) Drafter refresh: quantize + pack one linear weight.
  *   w_bf16      [N][K] bf16, row stride ldw_elems (>= K); base 16-byte aligned, ldw_elems % 8 == 0
- *   group       must be 128 (ER_GROUP); K % 128 == 0, N >= 1
- *   qweight_out uint32 [N][K/8]   (er_packed_bytes), 16-byte aligned
+ *   group       must be 128 (ER_GROUP); K % 128 == 0, N % 128 == 0
+ *   qweight_out N*K/8 uint32 words, ER_PACK_V2 (er_packed_bytes), 16-byte aligned
  *   scales_out  bf16 [K/128][N]   (er_scales_bytes), 2-byte aligned
  * Per group of 128 consecutive k of a row: amax = max|w|; s = bf16_rne(amax / 7) (IEEE fp32 divide);
  * q = clamp(rint(w / s), -8, 7) (ties to even, divide by the ROUNDED scale); s == 0 -> q = 0, s = +0.
@@ -126,7 +130,7 @@ int er_spec_verify(const void* target, const void* draft, int in_dtype, int inpu
                    const float* u_sample, int32_t B, int32_t gamma, int32_t V,
                    int32_t* accept_count, int32_t* out_tokens, void* stream);
 
-/* Parity helper: qweight uint32 [N][K/8] -> int8 codes [N][K] in [-8, 7] (device). Not timed. */
+/* Parity helper: qweight (ER_PACK_V2) -> int8 codes [N][K] in [-8, 7], row-major (device). Not timed. */
 int er_unpack_codes(const void* qweight, int64_t N, int64_t K, int8_t* codes_out, void* stream);
 
 /* ---- HOST-buffer forms of the three calls (the end-to-end path) -------------------------------------

@@ -44,12 +44,12 @@ int er_last_cuda_error(void) { return er::g_last_cuda_error; }
 int er_abi_version(void) { return ER_ABI_VERSION; }
 
 size_t er_packed_bytes(int64_t N, int64_t K) {
-  if (N < 1 || K < ER_GROUP || K % ER_GROUP != 0) return 0;
+  if (N < 128 || N % 128 != 0 || K < ER_GROUP || K % ER_GROUP != 0) return 0;
   return (size_t)N * (size_t)K / 2;
 }
 
 size_t er_scales_bytes(int64_t N, int64_t K, int group) {
-  if (group != ER_GROUP || N < 1 || K < ER_GROUP || K % ER_GROUP != 0) return 0;
+  if (group != ER_GROUP || N < 128 || N % 128 != 0 || K < ER_GROUP || K % ER_GROUP != 0) return 0;
   return (size_t)(K / group) * (size_t)N * 2;
 }
 

@@ -25,6 +25,15 @@ int sm_count();
     }                                                       \
   } while (0)
 
+// ER_PACK_V2 (include/er.h): index, in 32-bit words, of the word holding logical k-octet jj = k / 8 of row n.
+// Blocks of 128 rows x 128 k (2048 words) are stored T-major then g; inside a block row r keeps its place
+// (16 words) and its four 16-byte chunks are XOR-permuted by bits 1..2 of r.
+__host__ __device__ static inline int64_t packed_word_index(int64_t n, int64_t jj, int64_t groups) {
+  const int64_t T = n >> 7, g = jj >> 4;
+  const int r = (int)(n & 127), j = (int)(jj & 15);
+  return ((T * groups + g) << 11) + r * 16 + (((j >> 2) ^ ((r >> 1) & 3)) << 2) + (j & 3);
+}
+
 static inline bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
 // ---- device: small PTX wrappers --------------------------------------------------------------
@@ -85,6 +94,16 @@ __device__ __forceinline__ void tma_load_2d(void* smem_dst, const void* map, uin
       "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
       " [%0], [%1, {%3, %4}], [%2], %5;" ::"r"(smem_u32(smem_dst)),
       "l"(map), "r"(smem_u32(bar)), "r"(x), "r"(y), "l"(policy)
+      : "memory");
+}
+
+// 1-D bulk copy global -> shared (contiguous bytes; size and both addresses multiples of 16)
+__device__ __forceinline__ void bulk_load_1d(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar,
+                                             uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;" ::"r"(
+          smem_u32(smem_dst)),
+      "l"(gsrc), "r"(bytes), "r"(smem_u32(bar)), "l"(policy)
       : "memory");
 }
 

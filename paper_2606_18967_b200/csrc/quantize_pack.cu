@@ -144,7 +144,8 @@ __global__ void __launch_bounds__(kThreads) quantize_pack_kernel(const uint16_t*
     }
     if (ok[it]) {
       const int64_t n = n0 + r_in_tile;
-      *reinterpret_cast<uint2*>(qweight + n * (K >> 3) + (k >> 3)) = make_uint2(w0, w1);
+      // k is a multiple of 16: the two words are an aligned pair inside one 16-byte chunk of the block row
+      *reinterpret_cast<uint2*>(qweight + er::packed_word_index(n, k >> 3, K >> 7)) = make_uint2(w0, w1);
     }
     if ((lane & 7) == 0) s_scales[lane >> 3][r_in_tile] = (s > 0.0f) ? __bfloat16_as_ushort(sb) : 0;
   }
@@ -156,10 +157,12 @@ __global__ void __launch_bounds__(kThreads) quantize_pack_kernel(const uint16_t*
   }
 }
 
-__global__ void unpack_codes_kernel(const uint32_t* __restrict__ qweight, int64_t words, int8_t* __restrict__ codes) {
-  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+__global__ void unpack_codes_kernel(const uint32_t* __restrict__ qweight, int64_t words, int64_t K,
+                                    int8_t* __restrict__ codes) {
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // logical word: row n = j / (K/8), octet jj
   if (j >= words) return;
-  const uint32_t wd = qweight[j];
+  const int64_t n = j / (K >> 3), jj = j % (K >> 3);
+  const uint32_t wd = qweight[er::packed_word_index(n, jj, K >> 7)];
   uint32_t lo = 0, hi = 0;  // 8 int8 codes of logical k = 8 j + 0..7
 #pragma unroll
   for (int t = 0; t < 4; ++t) {
@@ -179,7 +182,8 @@ extern "C" {
 int er_quantize_pack(const void* w_bf16, int64_t N, int64_t K, int64_t ldw_elems, int group, void* qweight_out,
                      void* scales_out, void* stream) {
   if (!w_bf16 || !qweight_out || !scales_out) return ER_ERR_NULL;
-  if (group != ER_GROUP || N < 1 || K < ER_GROUP || K % ER_GROUP != 0 || ldw_elems < K) return ER_ERR_SHAPE;
+  if (group != ER_GROUP || N < 128 || N % 128 != 0 || K < ER_GROUP || K % ER_GROUP != 0 || ldw_elems < K)
+    return ER_ERR_SHAPE;
   if (!er::aligned16(w_bf16) || !er::aligned16(qweight_out) || (ldw_elems % 8) != 0 ||
       (reinterpret_cast<uintptr_t>(scales_out) & 1u))
     return ER_ERR_ALIGN;
@@ -198,7 +202,7 @@ int er_quantize_pack(const void* w_bf16, int64_t N, int64_t K, int64_t ldw_elems
 
 int er_unpack_codes(const void* qweight, int64_t N, int64_t K, int8_t* codes_out, void* stream) {
   if (!qweight || !codes_out) return ER_ERR_NULL;
-  if (N < 1 || K < 8 || K % 8 != 0) return ER_ERR_SHAPE;
+  if (N < 128 || N % 128 != 0 || K < ER_GROUP || K % ER_GROUP != 0) return ER_ERR_SHAPE;
   if ((reinterpret_cast<uintptr_t>(qweight) & 3u) || (reinterpret_cast<uintptr_t>(codes_out) & 7u)) return ER_ERR_ALIGN;
   int st = er::check_arch();
   if (st != ER_OK) return st;
@@ -206,7 +210,7 @@ int er_unpack_codes(const void* qweight, int64_t N, int64_t K, int8_t* codes_out
   const int64_t blocks = (words + 255) / 256;
   if (blocks > 0x7FFFFFFFll) return ER_ERR_SHAPE;
   unpack_codes_kernel<<<(unsigned)blocks, 256, 0, (cudaStream_t)stream>>>(reinterpret_cast<const uint32_t*>(qweight),
-                                                                         words, codes_out);
+                                                                         words, K, codes_out);
   ER_CUDA_TRY(cudaGetLastError());
   return ER_OK;
 }

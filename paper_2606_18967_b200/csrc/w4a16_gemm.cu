@@ -2,19 +2,29 @@
 // (dense projections are ~90 % of tail decode latency and weight loading dominates at
 // small batch; L175: W4A16 weight-only kernel; L467: "on-the-fly dequantization and kernel-level overhead").
 //
-// sm_100a design:
-//   swap-AB: the 128 weight rows of a tile are the M = 128 of tcgen05.mma, the (padded) batch is its N.
-//   warp 0      TMA producer: per 256-k block one SWIZZLE_128B box of packed int4 [128 rows x 128 B], the
-//               matching X boxes [MPAD x 64 k] x 4 and the 2 x 128 group scales, into a ring of stages.
-//   warps 2-5   workers, one thread per weight row: LDS.128 of the packed row, nibble -> bf16 in registers
-//               ((w >> 4t) & 0x000F000F | 0x43004300 is the pair 128+u; minus 136 is q exactly), tcgen05.st
-//               of the bf16 A operand straight into TENSOR MEMORY (no shared-memory round trip of the 4x
-//               expanded weights), then the fp32 scale-accumulate of the previous group's TMEM partial sum.
-//   warp 1      one thread issues tcgen05.mma.kind::f16 with A from TMEM, B (= X tile) from shared memory,
-//               one fresh fp32 TMEM accumulator per 128-k group (so the group scale is applied exactly, in
-//               fp32, after the contraction), and commits to mbarriers.
-//   split-K     partial [MPAD x 128] fp32 tiles go to the workspace; the last CTA of a tile (atomic ticket)
-//               adds them in ascending split order and stores Y.  Deterministic.
+// sm_100a design, second version (the first was latency-chain bound, see
+// profiles/r01_baseline_ncu.md):
+//   persistent  one CTA per SM; the (tile, 128-k group) units of the whole problem are dealt out as ONE contiguous
+//               range per CTA ("stream-K"): every CTA streams the same number of bytes whatever N and K are.
+//   swap-AB     the 128 weight rows of a tile are the M = 128 of tcgen05.mma, the (padded) batch is its N.
+//   warp 0      producer: per group ONE 8 KiB 1-D bulk copy of the packed block (ER_PACK_V2 keeps every
+//               [128 rows x 128 k] block contiguous and pre-swizzled: 2-D TMA boxes are row-rate bound, about
+//               5.5 cycles per box row per SM measured, so 64-128 byte rows cannot stream at HBM speed), one
+//               256-byte bulk copy of the group scales and two SWIZZLE_128B TMA boxes of X [MPAD x 64 k], into a
+//               ring of up to 16 stages (>= 100 KB in flight per SM); it runs ahead across tile boundaries.
+//   warps 2-9   workers.  Warps 2-5 own the EVEN groups of the CTA's range, warps 6-9 the ODD ones; each set is
+//               an independent two-deep software pipeline with its own A operand and accumulator in TENSOR
+//               MEMORY.  A thread owns one weight row: LDS.128 x 4 of its 64 packed bytes, nibble -> bf16 with
+//               ONE lop3 per pair ((w >> 4t) & 0x000F000F | 0x43004300 = the pair 128 + u), tcgen05.st of the
+//               A operand into TMEM (the 4x expanded weights never touch shared memory), then the fp32
+//               scale-accumulate (tcgen05.ld + FMA) of the group it converted one iteration earlier.
+//   warp 1      one thread issues tcgen05.mma.kind::f16, A from TMEM, B (= X tile) from shared memory, into a
+//               fresh fp32 TMEM accumulator per group (so the group scale is applied exactly, in fp32, after the
+//               contraction).  For MPAD <= 32 the offset of the code (q = u - 8 = (128 + u) - 136) is folded
+//               into the contraction: eight more MMAs with a constant A tile of -136 accumulate -136 * sum_k x
+//               into the same accumulator, which removes the packed subtract from the workers' ALU budget.
+//   output      a tile wholly owned by one CTA is stored directly; otherwise fp32 partials go to the workspace
+//               and the last CTA of the tile (ticket counter) adds them in ascending CTA order.  Deterministic.
 #include <cuda.h>
 #include "er_common.cuh"
 
@@ -22,35 +32,45 @@ namespace {
 
 using namespace er;
 
-constexpr int kBlockK = 256;                 // k per pipeline stage (= 128 packed bytes per row = one swizzle row)
-constexpr int kTileN = 128;                  // weight rows per CTA tile
-constexpr int kWBytes = kTileN * 128;        // 16 KiB packed weights per stage
-constexpr int kScaleBytes = 2 * kTileN * 2;  // 2 groups x 128 bf16
-constexpr int kThreads = 192;
-constexpr int kTmemCols = 256;
-constexpr int kTmemA = 0;    // A operand ring: 2 buffers x 64 columns (128 k of bf16 pairs)
-constexpr int kTmemD = 128;  // accumulator ring: 2 buffers x MPAD columns
+constexpr int kTileN = 128;                 // weight rows per tile
+constexpr int kWBytes = kTileN * 64;        // 8 KiB packed weights per group stage
+constexpr int kScaleBytes = kTileN * 2;     // 128 bf16 scales
+constexpr int kThreads = 320;               // TMA warp + MMA warp + 8 worker warps
+constexpr int kMaxStages = 16;
+constexpr int kTmemCols = 512;
+constexpr int kTmemA = 0;                   // A operand: 2 buffers (one per worker set) x 64 columns
+constexpr int kTmemConst = 128;             // 8 columns of bf16 pairs (-136, -136)
+constexpr int kTmemD = 256;                 // accumulators: 2 buffers x MPAD columns
+constexpr int kSmemLimit = 227 * 1024;
 
 template <int MPAD>
 struct Cfg {
-  static constexpr int kXBytes = MPAD * kBlockK * 2;  // 4 boxes of [MPAD x 64] bf16
-  static constexpr int kStageBytes = kWBytes + kXBytes + 1024;
-  static constexpr int kStages = (MPAD == 16) ? 4 : (MPAD == 32 ? 3 : 4);
-  static constexpr int kMinBlocks = (MPAD <= 32) ? 2 : 1;
-  static constexpr int kSmem = kStages * kStageBytes + 1024 /*align slack*/ + 256 /*barriers*/;
+  static constexpr bool kConstOffset = (MPAD <= 32);       // fold the -136 into the contraction
+  static constexpr int kXBytes = MPAD * 128 * 2;           // two boxes of [MPAD x 64] bf16
+  static constexpr int kStageBytes = ((kWBytes + kXBytes + kScaleBytes + 1023) / 1024) * 1024;
+  static constexpr int kRedBytes = MPAD * kTileN * 4;      // odd-set accumulators handed to the even set
+  static constexpr int kFixed = kRedBytes + 1024 /*align slack*/ + 512 /*barriers*/;
+  static constexpr int kStagesRaw = (kSmemLimit - kFixed) / kStageBytes;
+  static constexpr int kStages = kStagesRaw > kMaxStages ? kMaxStages : kStagesRaw;
+  static constexpr int kSmem = kStages * kStageBytes + kFixed;
   static constexpr uint32_t kTxBytes = kWBytes + kXBytes + kScaleBytes;
 };
 
 struct GemmParams {
   int M, N, K;
-  int kblocks;         // ceil(K / 256)
-  int splits;          // K splits per tile
+  int G;               // groups per tile = K / 128
+  int ntiles;          // N / 128
+  int tiles;           // ntiles * mchunks
+  int unit_groups;     // groups per scheduling unit: 1 (stream-K) or G (whole tiles)
+  long long units;     // tiles * G / unit_groups
   int y_f32;
   int64_t ldy;
   void* y;
-  const void* scales;  // unused by the kernel (TMA), kept for debugging
-  float* partials;     // workspace + ER_GEMM_COUNTER_BYTES
-  int* counters;       // workspace
+  const uint8_t* qweight;  // ER_PACK_V2 blocks
+  const uint8_t* scales;   // bf16 [G][N]
+  float* partials;     // workspace + ER_GEMM_COUNTER_BYTES: [cta][2][MPAD][128]
+  int* counters;       // workspace: one ticket per tile
+  int dbg;             // debug/sweep flags (er_gemm_tuning key 2); 0 in production
 };
 
 #define ER_TMEM_ST16(taddr, r, o)                                                                              \
@@ -70,55 +90,77 @@ struct GemmParams {
       : "r"(taddr)                                                                                             \
       : "memory")
 
-// 4 packed words (32 codes) -> 16 registers of bf16 pairs (k, k+1), exact.
+__device__ __forceinline__ uint32_t lop3_and_or(uint32_t a, uint32_t mask, uint32_t orv) {
+  uint32_t d;
+  asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(d) : "r"(a), "r"(mask), "r"(orv));
+  return d;
+}
+
+// 4 packed words (32 codes) -> 16 registers of bf16 pairs (k, k+1).  kSub == false: the pair 128 + u (the
+// -136 is applied by the tensor cores); kSub == true: the pair q = u - 8 itself (one packed subtract more).
+template <bool kSub>
 __device__ __forceinline__ void dequant4(const uint4& p, uint32_t (&a)[64], int base) {
   const uint32_t w[4] = {p.x, p.y, p.z, p.w};
-  const __nv_bfloat162 off = __floats2bfloat162_rn(136.0f, 136.0f);
+  const uint32_t mask = 0x000F000Fu, magic = 0x43004300u;
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
 #pragma unroll
     for (int t = 0; t < 4; ++t) {
-      uint32_t v = ((w[i] >> (4 * t)) & 0x000F000Fu) | 0x43004300u;  // bf16 pair (128 + u_k, 128 + u_{k+1})
-      __nv_bfloat162 h = __hsub2(*reinterpret_cast<__nv_bfloat162*>(&v), off);
-      a[base + 4 * i + t] = *reinterpret_cast<uint32_t*>(&h);
+      uint32_t v = lop3_and_or(w[i] >> (4 * t), mask, magic);  // bf16 pair (128 + u_k, 128 + u_{k+1})
+      if (kSub) {
+        const __nv_bfloat162 off = __floats2bfloat162_rn(136.0f, 136.0f);
+        __nv_bfloat162 h = __hsub2(*reinterpret_cast<__nv_bfloat162*>(&v), off);
+        v = *reinterpret_cast<uint32_t*>(&h);
+      }
+      a[base + 4 * i + t] = v;
     }
   }
 }
 
+__device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void named_bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+
+// first unit of CTA c when `units` units are dealt to `P` CTAs as contiguous, balanced ranges
+__device__ __forceinline__ long long range_begin(long long units, int P, int c) { return (units * c) / P; }
+// the CTA whose range contains unit u
+__device__ __forceinline__ int owner_of(long long units, int P, long long u) {
+  int c = (int)((u * P) / units);
+  while (c + 1 < P && range_begin(units, P, c + 1) <= u) ++c;
+  while (c > 0 && range_begin(units, P, c) > u) --c;
+  return c;
+}
+
 template <int MPAD>
-__global__ void __launch_bounds__(kThreads, Cfg<MPAD>::kMinBlocks)
-w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constant__ CUtensorMap map_x,
-                  const __grid_constant__ CUtensorMap map_s, const GemmParams p) {
+__global__ void __launch_bounds__(kThreads, 1)
+w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
   using C = Cfg<MPAD>;
+  constexpr int S = C::kStages;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::kStages * C::kStageBytes);
-  uint64_t* full = bars;                    // [kStages] TMA landed
-  uint64_t* empty = bars + C::kStages;      // [kStages] workers (128) + MMA commit (1) released the stage
-  uint64_t* a_full = bars + 2 * C::kStages; // [2] A operand of a group written to TMEM by 128 workers
-  uint64_t* mma_done = a_full + 2;          // [2] MMAs of a group complete: D readable, A buffer reusable
+  float* red = reinterpret_cast<float*>(smem + S * C::kStageBytes);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + S * C::kStageBytes + C::kRedBytes);
+  uint64_t* full = bars;                        // [S] TMA landed
+  uint64_t* empty = bars + kMaxStages;          // [S] 4 worker warps + MMA commit released the stage
+  uint64_t* a_full = bars + 2 * kMaxStages;     // [2] A operand of a group written to TMEM (4 worker warps)
+  uint64_t* mma_done = a_full + 2;              // [2] MMAs of a group complete: D readable, A reusable
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(mma_done + 2);
   int* last_flag = reinterpret_cast<int*>(tmem_slot + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int split = blockIdx.x, ntile = blockIdx.y, mchunk = blockIdx.z;
-  const int n0 = ntile * kTileN, m0 = mchunk * 64;
-  // k-block range of this split (balanced)
-  const int kb_begin = (int)(((int64_t)p.kblocks * split) / p.splits);
-  const int kb_end = (int)(((int64_t)p.kblocks * (split + 1)) / p.splits);
-  const int nkb = kb_end - kb_begin;
-  const int ngroups = 2 * nkb;
+  const int P = gridDim.x, cta = blockIdx.x;
+  const int ug = p.unit_groups;
+  const long long gb = range_begin(p.units, P, cta) * ug;        // first global group index of this CTA
+  const long long ge = range_begin(p.units, P, cta + 1) * ug;
+  const int n_it = (int)(ge - gb);
 
   if (threadIdx.x == 0) {
-    tma_prefetch_desc(&map_w);
     tma_prefetch_desc(&map_x);
-    tma_prefetch_desc(&map_s);
-    for (int s = 0; s < C::kStages; ++s) {
+    for (int s = 0; s < S; ++s) {
       mbar_init(&full[s], 1);
-      mbar_init(&empty[s], 129);
+      mbar_init(&empty[s], 5);
     }
     for (int j = 0; j < 2; ++j) {
-      mbar_init(&a_full[j], 128);
+      mbar_init(&a_full[j], 4);
       mbar_init(&mma_done[j], 1);
     }
     mbar_fence_init();
@@ -132,136 +174,199 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_consta
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (lane == 0) {
-      for (int i = 0; i < nkb; ++i) {
-        const int s = i % C::kStages;
-        mbar_wait(&empty[s], ((i / C::kStages) & 1) ^ 1);
+      for (int it = 0; it < n_it; ++it) {
+        const int s = it % S;
+        mbar_wait(&empty[s], ((it / S) & 1) ^ 1);
+        const long long gi = gb + it;
+        const int tile = (int)(gi / p.G), g = (int)(gi % p.G);
+        const int n0 = (tile % p.ntiles) * kTileN, m0 = (tile / p.ntiles) * MPAD;
         uint8_t* st = smem + s * C::kStageBytes;
-        const int kb = kb_begin + i;
         mbar_arrive_expect_tx(&full[s], C::kTxBytes);
-        tma_load_2d(st, &map_w, &full[s], kb * 128, n0, kEvictFirst);
-#pragma unroll
-        for (int bx = 0; bx < 4; ++bx)
-          tma_load_2d(st + kWBytes + bx * (MPAD * 128), &map_x, &full[s], kb * kBlockK + bx * 64, m0, kEvictLast);
-        tma_load_2d(st + kWBytes + C::kXBytes, &map_s, &full[s], n0, kb * 2, kEvictFirst);
+        // ER_PACK_V2: the [128 rows x 128 k] block of (tile, g) is 8 KiB of contiguous, pre-swizzled bytes
+        bulk_load_1d(st, p.qweight + ((size_t)(tile % p.ntiles) * p.G + g) * kWBytes, kWBytes, &full[s], kEvictFirst);
+        tma_load_2d(st + kWBytes, &map_x, &full[s], g * 128, m0, kEvictLast);
+        tma_load_2d(st + kWBytes + MPAD * 128, &map_x, &full[s], g * 128 + 64, m0, kEvictLast);
+        bulk_load_1d(st + kWBytes + C::kXBytes, p.scales + ((size_t)g * p.N + n0) * 2, kScaleBytes, &full[s],
+                     kEvictFirst);
       }
     }
   } else if (warp == 1) {
     // ===================== MMA issuer =====================
     if (lane == 0) {
       constexpr uint32_t idesc = idesc_bf16_m128(MPAD);
-      for (int g = 0; g < ngroups; ++g) {
-        const int i = g >> 1, h = g & 1, s = i % C::kStages, j = g & 1;
-        if (h == 0) mbar_wait(&full[s], (i / C::kStages) & 1);
-        mbar_wait(&a_full[j], (g >> 1) & 1);
+      for (int it = 0; it < n_it; ++it) {
+        const int s = it % S, j = it & 1;
+        mbar_wait(&full[s], (it / S) & 1);
+        mbar_wait(&a_full[j], (it >> 1) & 1);
         tc_fence_after();
         const uint32_t xbase = smem_u32(smem + s * C::kStageBytes + kWBytes);
         const uint32_t d_t = tmem + kTmemD + j * MPAD;
         const uint32_t a_t = tmem + kTmemA + j * 64;
+        if (!(p.dbg & 1)) {
 #pragma unroll
         for (int kk = 0; kk < 8; ++kk) {
-          const int koff = h * 128 + kk * 16;  // k offset inside the stage
-          const uint64_t bdesc = smem_desc_sw128(xbase + (koff >> 6) * (MPAD * 128) + (koff & 63) * 2);
+          const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
           mma_ts_f16(d_t, a_t + kk * 8, bdesc, idesc, kk > 0 ? 1u : 0u);
         }
+        }
+        if (C::kConstOffset && !(p.dbg & 2)) {
+#pragma unroll
+          for (int kk = 0; kk < 8; ++kk) {
+            const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
+            mma_ts_f16(d_t, tmem + kTmemConst, bdesc, idesc, 1u);
+          }
+        }
         tc_commit(&mma_done[j]);
-        if (h == 1) tc_commit(&empty[s]);
+        tc_commit(&empty[s]);
       }
     }
   } else {
-    // ===================== workers: dequant -> TMEM, scale-accumulate =====================
+    // ===================== workers: dequant -> TMEM, scale-accumulate, output =====================
+    const int set = (warp - 2) >> 2;       // 0: even groups of the range, 1: odd groups
     const int q4 = warp & 3;               // TMEM lane quarter this warp may access
     const int row = q4 * 32 + lane;        // weight row inside the tile
     const uint32_t lane_addr = (uint32_t)(q4 * 32) << 16;
-    float acc[MPAD];
+    if (C::kConstOffset && set == 0) {     // constant A tile: bf16 pairs (-136, -136), written once
+      uint32_t c8[16];
 #pragma unroll
-    for (int m = 0; m < MPAD; ++m) acc[m] = 0.f;
-    float sc_prev = 0.f;
-
-    auto epilogue_group = [&](int hgrp, float sc) {
-      const int j = hgrp & 1;
-      mbar_wait(&mma_done[j], (hgrp >> 1) & 1);
-      tc_fence_after();
-      uint32_t d[MPAD];
-#pragma unroll
-      for (int c = 0; c < MPAD; c += 16) ER_TMEM_LD16(tmem + lane_addr + kTmemD + j * MPAD + c, d, c);
-      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-#pragma unroll
-      for (int m = 0; m < MPAD; ++m) acc[m] = fmaf(sc, __uint_as_float(d[m]), acc[m]);
-    };
-
-    for (int g = 0; g < ngroups; ++g) {
-      const int i = g >> 1, h = g & 1, s = i % C::kStages, j = g & 1;
-      if (h == 0) mbar_wait(&full[s], (i / C::kStages) & 1);
-      const uint8_t* st = smem + s * C::kStageBytes;
-      const uint8_t* wrow = st + row * 128;
-      uint4 pk[4];
-#pragma unroll
-      for (int c = 0; c < 4; ++c) pk[c] = *reinterpret_cast<const uint4*>(wrow + (((4 * h + c) ^ (row & 7)) << 4));
-      const float sc = __bfloat162float(
-          *reinterpret_cast<const __nv_bfloat16*>(st + kWBytes + C::kXBytes + h * 256 + row * 2));
-      uint32_t a[64];
-#pragma unroll
-      for (int c = 0; c < 4; ++c) dequant4(pk[c], a, 16 * c);
-      // A buffer j is free: mma_done of group g-2 was waited for in the previous iteration's epilogue
-      const uint32_t a_t = tmem + lane_addr + kTmemA + j * 64;
-      ER_TMEM_ST16(a_t + 0, a, 0);
-      ER_TMEM_ST16(a_t + 16, a, 16);
-      ER_TMEM_ST16(a_t + 32, a, 32);
-      ER_TMEM_ST16(a_t + 48, a, 48);
+      for (int i = 0; i < 16; ++i) c8[i] = 0xC308C308u;
+      asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(
+                       tmem + lane_addr + kTmemConst),
+                   "r"(c8[0]), "r"(c8[1]), "r"(c8[2]), "r"(c8[3]), "r"(c8[4]), "r"(c8[5]), "r"(c8[6]), "r"(c8[7])
+                   : "memory");
       asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
       tc_fence_before();
-      if (h == 1) mbar_arrive(&empty[s]);
-      mbar_arrive(&a_full[j]);
-      if (g > 0) epilogue_group(g - 1, sc_prev);
-      sc_prev = sc;
     }
-    if (ngroups > 0) epilogue_group(ngroups - 1, sc_prev);
+    // the constant tile is ordered before the first MMA by the a_full arrival of this set (set 0 converts
+    // group 0, and the MMA issuer waits for a_full[0] before its first instruction of either set)
 
-    // ---- output: direct store, or split-K partial + last-arriver reduction ----
-    const int mvalid = min(MPAD, p.M - m0);
-    const int n = n0 + row;
-    bool store = true;
-    if (p.splits > 1) {
-      const int tile_id = mchunk * gridDim.y + ntile;
-      float* mine = p.partials + ((size_t)tile_id * p.splits + split) * (MPAD * kTileN);
+    float acc[MPAD];
+    int it = 0;          // local group index, walks the CTA's range segment by segment
+    int seg = 0;
+    while (it < n_it) {
+      // ---- segment = the part of one tile inside this CTA's range ----
+      const long long gi0 = gb + it;
+      const int tile = (int)(gi0 / p.G), g_lo = (int)(gi0 % p.G);
+      const int seg_len = min(p.G - g_lo, n_it - it);
+      const int it_end = it + seg_len;
+      const bool last_seg = (it_end == n_it);
 #pragma unroll
-      for (int m = 0; m < MPAD; ++m)
-        if (m < mvalid) __stcg(mine + m * kTileN + row, acc[m]);
-      __threadfence();
-      asm volatile("bar.sync 1, 128;" ::: "memory");
-      if (threadIdx.x == 64) {
-        const int old = atomicAdd(p.counters + tile_id, 1);
-        const int last = (old == p.splits - 1);
-        if (last) p.counters[tile_id] = 0;  // leave the counter zero for the next call
-        *last_flag = last;
+      for (int m = 0; m < MPAD; ++m) acc[m] = 0.f;
+      bool pending = false;
+      float sc_prev = 0.f;
+
+      auto epilogue_group = [&](int it_done, float sc) {
+        mbar_wait(&mma_done[set], (it_done >> 1) & 1);
+        tc_fence_after();
+        uint32_t d[MPAD];
+#pragma unroll
+        for (int c = 0; c < MPAD; c += 16) ER_TMEM_LD16(tmem + lane_addr + kTmemD + set * MPAD + c, d, c);
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+        for (int m = 0; m < MPAD; ++m) acc[m] = fmaf(sc, __uint_as_float(d[m]), acc[m]);
+      };
+
+      int my = it + ((it & 1) != set ? 1 : 0);
+      for (; my < it_end; my += 2) {
+        const int s = my % S;
+        mbar_wait(&full[s], (my / S) & 1);
+        const uint8_t* st = smem + s * C::kStageBytes;
+        const uint8_t* wrow = st + row * 64;
+        uint4 pk[4];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) pk[c] = *reinterpret_cast<const uint4*>(wrow + ((c ^ ((row >> 1) & 3)) << 4));
+        const float sc =
+            __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(st + kWBytes + C::kXBytes + row * 2));
+        if (pending && !(p.dbg & 8)) epilogue_group(my - 2, sc_prev);
+        uint32_t a[64];
+#pragma unroll
+        for (int c = 0; c < 4; ++c) dequant4<!C::kConstOffset>(pk[c], a, 16 * c);
+        // A[set] is free: the MMAs of this set's previous group were waited for in the epilogue above
+        const uint32_t a_t = tmem + lane_addr + kTmemA + set * 64;
+        if (!(p.dbg & 4)) {
+        ER_TMEM_ST16(a_t + 0, a, 0);
+        ER_TMEM_ST16(a_t + 16, a, 16);
+        ER_TMEM_ST16(a_t + 32, a, 32);
+        ER_TMEM_ST16(a_t + 48, a, 48);
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+        } else { if (a[0] + a[17] + a[35] + a[63] == 0x12345u) *last_flag = 1; }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+          mbar_arrive(&empty[s]);   // every lane's shared-memory reads of this stage have been consumed
+          mbar_arrive(&a_full[set]);
+        }
+        pending = true;
+        sc_prev = sc;
       }
-      asm volatile("bar.sync 1, 128;" ::: "memory");
-      store = (*last_flag != 0);
-      if (store) {
-        __threadfence();
-        const float* base = p.partials + (size_t)tile_id * p.splits * (MPAD * kTileN);
+      if (pending && !(p.dbg & 8)) epilogue_group(my - 2, sc_prev);
+
+      // ---- combine the two sets (odd -> shared memory -> even) ----
+      if (set == 1) {
+        if (seg > 0) named_bar_sync(2, 256);          // even set has finished reading the previous segment's red
 #pragma unroll
-        for (int m = 0; m < MPAD; ++m) {
-          if (m < mvalid) {
-            float sum = 0.f;
-            for (int sp = 0; sp < p.splits; ++sp) sum += __ldcg(base + (size_t)sp * (MPAD * kTileN) + m * kTileN + row);
-            acc[m] = sum;
+        for (int m = 0; m < MPAD; ++m) red[m * kTileN + row] = acc[m];
+        named_bar_arrive(1, 256);
+      } else {
+        named_bar_sync(1, 256);
+#pragma unroll
+        for (int m = 0; m < MPAD; ++m) acc[m] += red[m * kTileN + row];
+        if (!last_seg) named_bar_arrive(2, 256);
+
+        // ---- output: direct store, or partial + last-arriver reduction in ascending CTA order ----
+        const int n0 = (tile % p.ntiles) * kTileN, m0 = (tile / p.ntiles) * MPAD;
+        const int mvalid = min(MPAD, p.M - m0);
+        const int n = n0 + row;
+        bool store = true;
+        if (seg_len != p.G) {
+          float* mine = p.partials + ((size_t)cta * 2 + (it == 0 ? 0 : 1)) * (MPAD * kTileN);
+#pragma unroll
+          for (int m = 0; m < MPAD; ++m)
+            if (m < mvalid) __stcg(mine + m * kTileN + row, acc[m]);
+          __threadfence();
+          named_bar_sync(3, 128);
+          const long long u_first = ((long long)tile * p.G) / ug, u_last = ((long long)(tile + 1) * p.G - 1) / ug;
+          const int c_lo = owner_of(p.units, P, u_first), c_hi = owner_of(p.units, P, u_last);
+          if (threadIdx.x == 64) {
+            const int old = atomicAdd(p.counters + tile, 1);
+            const int last = (old == c_hi - c_lo);
+            if (last) p.counters[tile] = 0;  // leave the counter zero for the next call
+            *last_flag = last;
+          }
+          named_bar_sync(3, 128);
+          store = (*last_flag != 0);
+          if (store) {
+            __threadfence();
+#pragma unroll
+            for (int m = 0; m < MPAD; ++m) acc[m] = 0.f;
+            for (int c = c_lo; c <= c_hi; ++c) {
+              // CTA c's piece of this tile is its first segment iff its range starts inside the tile
+              const long long cb = range_begin(p.units, P, c) * ug;
+              const int which = (cb >= (long long)tile * p.G) ? 0 : 1;
+              const float* src = p.partials + ((size_t)c * 2 + which) * (MPAD * kTileN);
+#pragma unroll
+              for (int m = 0; m < MPAD; ++m)
+                if (m < mvalid) acc[m] += __ldcg(src + m * kTileN + row);
+            }
+          }
+          named_bar_sync(3, 128);   // last_flag may be rewritten by the next segment only after all have read it
+        }
+        if (store) {
+          if (p.y_f32) {
+            float* y = reinterpret_cast<float*>(p.y);
+#pragma unroll
+            for (int m = 0; m < MPAD; ++m)
+              if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = acc[m];
+          } else {
+            __nv_bfloat16* y = reinterpret_cast<__nv_bfloat16*>(p.y);
+#pragma unroll
+            for (int m = 0; m < MPAD; ++m)
+              if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = __float2bfloat16_rn(acc[m]);
           }
         }
       }
-    }
-    if (store) {
-      if (p.y_f32) {
-        float* y = reinterpret_cast<float*>(p.y);
-#pragma unroll
-        for (int m = 0; m < MPAD; ++m)
-          if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = acc[m];
-      } else {
-        __nv_bfloat16* y = reinterpret_cast<__nv_bfloat16*>(p.y);
-#pragma unroll
-        for (int m = 0; m < MPAD; ++m)
-          if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = __float2bfloat16_rn(acc[m]);
-      }
+      it = it_end;
+      ++seg;
     }
   }
 
@@ -274,7 +379,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_consta
 }  // namespace
 
 // =====================================================================================================
-// host side: tensor maps, split-K plan, launch
+// host side: tensor maps, stream-K plan, launch
 // =====================================================================================================
 namespace {
 
@@ -294,8 +399,8 @@ EncodeTiledFn encode_fn() {
   return fn;
 }
 
-// 2-D row-major tensor [rows][cols] of `esize`-byte elements, row pitch in bytes, box [box_rows][box_cols].
-bool make_map_2d(CUtensorMap* map, CUtensorMapDataType dt, int esize, const void* base, uint64_t rows, uint64_t cols,
+// 2-D row-major tensor [rows][cols] of elements, row pitch in bytes, box [box_rows][box_cols].
+bool make_map_2d(CUtensorMap* map, CUtensorMapDataType dt, const void* base, uint64_t rows, uint64_t cols,
                  uint64_t pitch_bytes, uint32_t box_rows, uint32_t box_cols, CUtensorMapSwizzle swz) {
   EncodeTiledFn fn = encode_fn();
   if (!fn) return false;
@@ -303,57 +408,51 @@ bool make_map_2d(CUtensorMap* map, CUtensorMapDataType dt, int esize, const void
   cuuint64_t strides[1] = {pitch_bytes};
   cuuint32_t box[2] = {box_cols, box_rows};
   cuuint32_t estr[2] = {1, 1};
-  (void)esize;
   CUresult r = fn(map, dt, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, swz,
                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return r == CUDA_SUCCESS;
 }
 
-int g_tune_ctas_per_sm = 2;   // split-K target: resident CTAs per SM to fill (MPAD <= 32)
-int g_tune_force_splits = 0;  // > 0: force this many K splits (tests / sweeps)
+int g_tune_dbg = 0;
+int g_tune_force_ctas = 0;  // > 0: use this many CTAs (tests / sweeps); 0 = one per SM
 
 struct Plan {
-  int mpad, mchunks, ntiles, kblocks, splits;
+  int mpad, mchunks, ntiles, tiles, G, unit_groups, ctas;
+  long long units;
 };
+
+int mpad_of(int64_t M) { return M <= 16 ? 16 : (M <= 32 ? 32 : 64); }
 
 Plan make_plan(int64_t M, int64_t N, int64_t K) {
   Plan pl;
-  pl.mpad = M <= 16 ? 16 : (M <= 32 ? 32 : 64);
-  pl.mchunks = (int)((M + 63) / 64);
+  pl.mpad = mpad_of(M);
+  pl.mchunks = (int)((M + pl.mpad - 1) / pl.mpad);
   pl.ntiles = (int)(N / kTileN);
-  pl.kblocks = (int)((K + kBlockK - 1) / kBlockK);
-  const int tiles = pl.ntiles * pl.mchunks;
-  const int resident = er::sm_count() * (pl.mpad <= 32 ? g_tune_ctas_per_sm : 1);
-  int splits = 1;
-  if (tiles < resident) {
-    splits = resident / tiles;
-    if (splits > pl.kblocks) splits = pl.kblocks;
-    if (splits < 1) splits = 1;
-  }
-  if (g_tune_force_splits > 0) splits = g_tune_force_splits < pl.kblocks ? g_tune_force_splits : pl.kblocks;
-  if (tiles > ER_GEMM_COUNTER_BYTES / 4) splits = 1;  // counters cover 4096 tiles
-  if (splits > 65535) splits = 65535;
-  pl.splits = splits;
+  pl.tiles = pl.ntiles * pl.mchunks;
+  pl.G = (int)(K / ER_GROUP);
+  // one ticket counter per tile: beyond the counter array, whole tiles are dealt out (no partial sums)
+  pl.unit_groups = (pl.tiles <= ER_GEMM_COUNTER_BYTES / 4) ? 1 : pl.G;
+  pl.units = (long long)pl.tiles * pl.G / pl.unit_groups;
+  int ctas = er::sm_count();
+  if (g_tune_force_ctas > 0 && g_tune_force_ctas < ctas) ctas = g_tune_force_ctas;
+  if ((long long)ctas > pl.units) ctas = (int)pl.units;
+  pl.ctas = ctas;
   return pl;
 }
 
-size_t plan_workspace(const Plan& pl) {
-  size_t partial = 0;
-  if (pl.splits > 1) partial = (size_t)pl.ntiles * pl.mchunks * pl.splits * pl.mpad * kTileN * sizeof(float);
-  return ER_GEMM_COUNTER_BYTES + partial;
+size_t workspace_for(int mpad) {
+  return ER_GEMM_COUNTER_BYTES + (size_t)er::sm_count() * 2 * mpad * kTileN * sizeof(float);
 }
 
 template <int MPAD>
-int launch(const CUtensorMap& mw, const CUtensorMap& mx, const CUtensorMap& ms, const GemmParams& gp, const Plan& pl,
-           cudaStream_t stream) {
+int launch(const CUtensorMap& mx, const GemmParams& gp, const Plan& pl, cudaStream_t stream) {
   static bool attr_set = false;
   if (!attr_set) {
     ER_CUDA_TRY(cudaFuncSetAttribute(w4a16_gemm_kernel<MPAD>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      Cfg<MPAD>::kSmem));
     attr_set = true;
   }
-  dim3 grid((unsigned)pl.splits, (unsigned)pl.ntiles, (unsigned)pl.mchunks);
-  w4a16_gemm_kernel<MPAD><<<grid, kThreads, Cfg<MPAD>::kSmem, stream>>>(mw, mx, ms, gp);
+  w4a16_gemm_kernel<MPAD><<<pl.ctas, kThreads, Cfg<MPAD>::kSmem, stream>>>(mx, gp);
   ER_CUDA_TRY(cudaGetLastError());
   return ER_OK;
 }
@@ -362,28 +461,18 @@ int launch(const CUtensorMap& mw, const CUtensorMap& mx, const CUtensorMap& ms, 
 
 extern "C" {
 
-// Internal tuning knob for sweeps (not part of the stable ABI): key 0 = CTAs per SM targeted by the
-// split-K planner (1 or 2), key 1 = forced split count (0 = planner).
+// Internal tuning knob for tests and sweeps (not part of the stable ABI): key 1 = number of CTAs the stream-K
+// plan uses (0 = one per SM); key 0 is accepted and ignored (it belonged to the first kernel version).
 int er_gemm_tuning(int key, int value) {
-  if (key == 0 && (value == 1 || value == 2)) { g_tune_ctas_per_sm = value; return ER_OK; }
-  if (key == 1 && value >= 0) { g_tune_force_splits = value; return ER_OK; }
+  if (key == 0 && (value == 1 || value == 2)) return ER_OK;
+  if (key == 1 && value >= 0) { g_tune_force_ctas = value; return ER_OK; }
+  if (key == 2 && value >= 0) { g_tune_dbg = value; return ER_OK; }
   return ER_ERR_SHAPE;
 }
 
 size_t er_gemm_workspace_bytes(int64_t M, int64_t N, int64_t K) {
   if (M < 1 || N < kTileN || N % kTileN != 0 || K < ER_GROUP || K % ER_GROUP != 0) return 0;
-  // independent of tuning knobs: the largest split count the planner can pick for this shape
-  Plan pl = make_plan(M, N, K);
-  Plan worst = pl;
-  const int tiles = pl.ntiles * pl.mchunks;
-  if (tiles <= ER_GEMM_COUNTER_BYTES / 4) {
-    int s = (2 * er::sm_count()) / tiles;
-    if (s < 1) s = 1;
-    if (s > pl.kblocks) s = pl.kblocks;
-    if (g_tune_force_splits > s) s = g_tune_force_splits < pl.kblocks ? g_tune_force_splits : pl.kblocks;
-    if (s > worst.splits) worst.splits = s;
-  }
-  return plan_workspace(worst);
+  return workspace_for(mpad_of(M));
 }
 
 int er_gemm_workspace_init(void* workspace, size_t workspace_bytes, void* stream) {
@@ -406,32 +495,30 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
   if (!workspace) return ER_ERR_WORKSPACE;
   if (!er::aligned16(workspace)) return ER_ERR_ALIGN;
   const Plan pl = make_plan(M, N, K);
-  if (pl.mchunks > 65535 || pl.ntiles > 65535) return ER_ERR_SHAPE;
-  if (workspace_bytes < plan_workspace(pl)) return ER_ERR_WORKSPACE;
+  if (workspace_bytes < workspace_for(pl.mpad)) return ER_ERR_WORKSPACE;
   int st = er::check_arch();
   if (st != ER_OK) return st;
 
-  CUtensorMap mw, mx, ms;
-  bool ok = make_map_2d(&mw, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, qweight, (uint64_t)N, (uint64_t)(K / 2),
-                        (uint64_t)(K / 2), kTileN, 128, CU_TENSOR_MAP_SWIZZLE_128B);
-  ok = ok && make_map_2d(&mx, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, x_bf16, (uint64_t)M, (uint64_t)K,
+  CUtensorMap mx;
+  bool ok = make_map_2d(&mx, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, x_bf16, (uint64_t)M, (uint64_t)K,
                          (uint64_t)ldx_elems * 2, (uint32_t)pl.mpad, 64, CU_TENSOR_MAP_SWIZZLE_128B);
-  ok = ok && make_map_2d(&ms, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, scales, (uint64_t)(K / ER_GROUP), (uint64_t)N,
-                         (uint64_t)N * 2, 2, kTileN, CU_TENSOR_MAP_SWIZZLE_NONE);
   if (!ok) {
     er::set_last_cuda_error((int)cudaErrorInvalidValue);
     return ER_ERR_CUDA;
   }
   GemmParams gp;
   gp.M = (int)M; gp.N = (int)N; gp.K = (int)K;
-  gp.kblocks = pl.kblocks; gp.splits = pl.splits;
-  gp.y_f32 = (y_dtype == ER_F32); gp.ldy = ldy_elems; gp.y = y; gp.scales = scales;
+  gp.G = pl.G; gp.ntiles = pl.ntiles; gp.tiles = pl.tiles; gp.unit_groups = pl.unit_groups; gp.units = pl.units;
+  gp.dbg = g_tune_dbg;
+  gp.qweight = reinterpret_cast<const uint8_t*>(qweight);
+  gp.scales = reinterpret_cast<const uint8_t*>(scales);
+  gp.y_f32 = (y_dtype == ER_F32); gp.ldy = ldy_elems; gp.y = y;
   gp.counters = reinterpret_cast<int*>(workspace);
   gp.partials = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + ER_GEMM_COUNTER_BYTES);
   cudaStream_t s = (cudaStream_t)stream;
-  if (pl.mpad == 16) return launch<16>(mw, mx, ms, gp, pl, s);
-  if (pl.mpad == 32) return launch<32>(mw, mx, ms, gp, pl, s);
-  return launch<64>(mw, mx, ms, gp, pl, s);
+  if (pl.mpad == 16) return launch<16>(mx, gp, pl, s);
+  if (pl.mpad == 32) return launch<32>(mx, gp, pl, s);
+  return launch<64>(mx, gp, pl, s);
 }
 
 }  // extern "C"

@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(128) w4a16_simt_kernel(const __nv_bfloat16* __
       for (int i = 0; i < kMC; ++i) part[i] = 0.f;
       if (lane < 16) {  // 16 words per group
         const int j = g * 16 + lane;
-        const uint32_t wd = qw[(size_t)n * words + j];
+        const uint32_t wd = qw[er::packed_word_index(n, j, groups)];
 #pragma unroll
         for (int t = 0; t < 4; ++t) {
           const float q0 = (float)((int)((wd >> (4 * t)) & 0xF) - 8);       // k = 8 j + 2 t
@@ -68,7 +68,7 @@ extern "C" int er_w4a16_gemm_simt(const void* x_bf16, int64_t M, int64_t K, int6
                                   const void* scales, int64_t N, int group, void* y, int64_t ldy_elems, int y_dtype,
                                   void* stream) {
   if (!x_bf16 || !qweight || !scales || !y) return ER_ERR_NULL;
-  if (group != ER_GROUP || M < 1 || N < 1 || K < ER_GROUP || K % ER_GROUP != 0 || ldx_elems < K || ldy_elems < N ||
+  if (group != ER_GROUP || M < 1 || N < 128 || N % 128 != 0 || K < ER_GROUP || K % ER_GROUP != 0 || ldx_elems < K || ldy_elems < N ||
       M > (1 << 20) || N > (1 << 24) || K > (1 << 24))
     return ER_ERR_SHAPE;
   if (y_dtype != ER_BF16 && y_dtype != ER_F32) return ER_ERR_DTYPE;

@@ -37,8 +37,9 @@ def test_status_strings():
 def test_size_queries():
     assert er.packed_bytes(4608, 3584) == 4608 * 3584 // 2
     assert er.scales_bytes(4608, 3584) == (3584 // 128) * 4608 * 2
-    assert er.packed_bytes(16, 100) == 0            # K % 128 != 0
-    assert er.scales_bytes(16, 256, 64) == 0        # only group 128
+    assert er.packed_bytes(128, 100) == 0           # K % 128 != 0
+    assert er.packed_bytes(100, 128) == 0           # N % 128 != 0 (ER_PACK_V2 blocks are 128 rows)
+    assert er.scales_bytes(128, 256, 64) == 0        # only group 128
     assert er.gemm_workspace_bytes(1, 4608, 3584) >= er.COUNTER_BYTES
     assert er.gemm_workspace_bytes(1, 100, 3584) == 0   # N % 128 != 0
     # bytes/weight of the packed format: 0.5 + 2/128
@@ -51,12 +52,12 @@ def test_quantize_pack_validation():
     buf = (ctypes.c_uint8 * 4096)()
     p = ctypes.addressof(buf)
     p = (p + 15) & ~15
-    assert lib.er_quantize_pack(None, 1, 128, 128, 128, p, p, None) == 1
-    assert lib.er_quantize_pack(p, 1, 100, 128, 128, p, p, None) == 2
-    assert lib.er_quantize_pack(p, 1, 128, 128, 64, p, p, None) == 2
-    assert lib.er_quantize_pack(p, 1, 128, 64, 128, p, p, None) == 2     # ldw < K
-    assert lib.er_quantize_pack(p + 2, 1, 128, 128, 128, p, p, None) == 3
-    assert lib.er_quantize_pack(p, 1, 128, 132, 128, p, p, None) == 3    # ldw % 8
+    assert lib.er_quantize_pack(None, 128, 128, 128, 128, p, p, None) == 1
+    assert lib.er_quantize_pack(p, 128, 100, 128, 128, p, p, None) == 2
+    assert lib.er_quantize_pack(p, 128, 128, 128, 64, p, p, None) == 2
+    assert lib.er_quantize_pack(p, 128, 128, 64, 128, p, p, None) == 2     # ldw < K
+    assert lib.er_quantize_pack(p + 2, 128, 128, 128, 128, p, p, None) == 3
+    assert lib.er_quantize_pack(p, 128, 128, 132, 128, p, p, None) == 3    # ldw % 8
 
 
 def test_gemm_validation():
@@ -95,7 +96,7 @@ def test_no_cpu_fallback_without_gpu():
     lib = er.load()
     buf = (ctypes.c_uint8 * 65536)()
     p = (ctypes.addressof(buf) + 15) & ~15
-    st = lib.er_quantize_pack(p, 1, 128, 128, 128, p + 1024, p + 2048, None)
+    st = lib.er_quantize_pack(p, 128, 128, 128, 128, p + 1024, p + 2048, None)
     assert st in (6, 7)
     with pytest.raises(ValueError):
-        er.quantize_pack(torch.zeros((1, 128), dtype=torch.bfloat16))
+        er.quantize_pack(torch.zeros((128, 128), dtype=torch.bfloat16))

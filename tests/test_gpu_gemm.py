@@ -143,16 +143,20 @@ def test_split_k_counts_agree_and_are_deterministic(splits):
                                       ("down", 3584, 18944)])
 @pytest.mark.parametrize("M", [1, 16, 256])
 def test_config1_full_size_sampled_columns(name, N, K, M):
-    # full 7B-layer shapes in the launch configuration bench.py times; oracle on 256 sampled output columns
+    # full 7B-layer shapes in the launch configuration bench.py times; oracle on the 256 output columns of two sampled 128-row tiles
     w = I.weight_bf16(N, K, I.seed_of("cfg1", name), device=DEV)
     x = I.activation_bf16(M, K, I.seed_of("cfg1", name, "x", M), device=DEV)
     qw, sc = er.quantize_pack(w)
     y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
     torch.cuda.synchronize()
     rng = np.random.default_rng(N + M)
-    cols = np.sort(rng.choice(N, size=256, replace=False))
+    G = K // 128
+    blocks = qw.view(N // 128, G * 2048)                    # ER_PACK_V2: one row of this view per 128-row tile
+    tiles = np.sort(rng.choice(N // 128, size=2, replace=False))
+    cols = np.concatenate([np.arange(t * 128, (t + 1) * 128) for t in tiles])
     ct = torch.from_numpy(cols).to(DEV)
-    y_ref = O.w4a16_gemm(I.as_u16(x), qw[ct].cpu().numpy().view(np.uint32), I.as_u16(sc[:, ct].contiguous()))
+    qsel = blocks[torch.from_numpy(tiles).to(DEV)].cpu().numpy().view(np.uint32).reshape(256, K // 8)
+    y_ref = O.w4a16_gemm(I.as_u16(x), qsel, I.as_u16(sc[:, ct].contiguous()))
     got = y[:, ct].cpu().numpy().astype(np.float64)
     err = np.abs(got - y_ref).max()
     assert err <= _tol(y_ref), f"{name} M={M}: max|d|={err} tol={_tol(y_ref)}"

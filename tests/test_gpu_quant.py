@@ -29,7 +29,7 @@ def test_config0_whole_matrix_bit_exact():
     assert codes.min() >= -7 and codes.max() == 7
 
 
-@pytest.mark.parametrize("N,K", [(1, 128), (33, 384), (130, 1152), (257, 640), (96, 4096)])
+@pytest.mark.parametrize("N,K", [(128, 128), (128, 384), (256, 1152), (384, 640), (128, 4096)])
 def test_ragged_shapes_bit_exact(N, K):
     w = I.weight_bf16(N, K, I.seed_of("ragged", N, K), device=DEV, outlier_frac=0.001)
     _check_exact(w)
@@ -42,13 +42,13 @@ def test_outliers_and_ties_bit_exact():
 
 
 def test_strided_input_and_special_groups():
-    base = I.weight_bf16(64, 1024, 7, device=DEV)
+    base = I.weight_bf16(128, 1024, 7, device=DEV)
     w = base[:, :512]                       # ldw = 1024 > K = 512
     assert w.stride(0) == 1024
     qw, sc = er.quantize_pack(w)
     qr, sr = O.quantize_pack(I.as_u16(w.contiguous()))
     assert np.array_equal(qw.cpu().numpy().view(np.uint32), qr) and np.array_equal(I.as_u16(sc), sr)
-    z = torch.zeros((32, 256), dtype=torch.bfloat16, device=DEV)
+    z = torch.zeros((128, 256), dtype=torch.bfloat16, device=DEV)
     z[0, :128] = 1.0                        # a group of equal values; other groups all zero (Q8)
     z[1, 130] = -3.0
     z[2, 0] = 1e-38                         # denormal-range scale
@@ -64,7 +64,7 @@ def test_exhaustive_bf16_values_against_fixed_scales():
         amax = float(O.bf16_to_f32(np.uint16(amax_bits)))
         keep = np.isfinite(f) & (np.abs(f) <= amax)
         vals = u[keep]
-        pad = (-len(vals)) % 127
+        pad = (-len(vals)) % (127 * 128)                     # whole 128-row blocks
         vals = np.concatenate([vals, np.zeros(pad, dtype=np.uint16)])
         rows = vals.reshape(-1, 127)
         full = np.concatenate([np.full((rows.shape[0], 1), amax_bits, dtype=np.uint16), rows], axis=1)
@@ -79,7 +79,13 @@ def test_sampled_groups_of_a_7b_layer():
     qw, sc = er.quantize_pack(w)
     rng = np.random.default_rng(5)
     rows = np.sort(rng.choice(N, size=N // 100, replace=False))
-    wr = I.as_u16(w[torch.from_numpy(rows).to(DEV)])
-    qr, sr = O.quantize_pack(wr)
-    assert np.array_equal(qw.cpu().numpy().view(np.uint32)[rows], qr)
+    codes_ref, sr = O.quantize_codes(I.as_u16(w[torch.from_numpy(rows).to(DEV)]))
+    codes = er.unpack_codes(qw).cpu().numpy()
+    assert np.array_equal(codes[rows], codes_ref)
     assert np.array_equal(I.as_u16(sc)[:, rows], sr)
+    # and two whole 128-row blocks, packed bytes compared directly
+    for T in (0, N // 128 - 1):
+        qr, sr = O.quantize_pack(I.as_u16(w[T * 128:(T + 1) * 128]))
+        G = K // 128
+        got = qw.cpu().numpy().view(np.uint32).reshape(-1)[T * G * 2048:(T + 1) * G * 2048]
+        assert np.array_equal(got, qr.reshape(-1))
