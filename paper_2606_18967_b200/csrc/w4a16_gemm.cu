@@ -7,18 +7,18 @@
 //   persistent  one CTA per SM; the (tile, 128-k group) units of the whole problem are dealt out as ONE contiguous
 //               range per CTA ("stream-K"): every CTA streams the same number of bytes whatever N and K are.
 //   swap-AB     the 128 weight rows of a tile are the M = 128 of tcgen05.mma, the (padded) batch is its N.
-//   warp 0      producer: per group ONE 8 KiB 1-D bulk copy of the packed block (ER_PACK_V2 keeps every
+//   warps 0-1   producers (even / odd groups), one thread each: per group ONE 8 KiB 1-D bulk copy of the packed block (ER_PACK_V2 keeps every
 //               [128 rows x 128 k] block contiguous and pre-swizzled: 2-D TMA boxes are row-rate bound, about
 //               5.5 cycles per box row per SM measured, so 64-128 byte rows cannot stream at HBM speed), one
 //               256-byte bulk copy of the group scales and two SWIZZLE_128B TMA boxes of X [MPAD x 64 k], into a
 //               ring of up to 16 stages (>= 100 KB in flight per SM); it runs ahead across tile boundaries.
-//   warps 2-9   workers.  Warps 2-5 own the EVEN groups of the CTA's range, warps 6-9 the ODD ones; each set is
+//   warps 4-11  workers.  Warps 4-7 own the EVEN groups of the CTA's range, warps 8-11 the ODD ones; each set is
 //               an independent two-deep software pipeline with its own A operand and accumulator in TENSOR
 //               MEMORY.  A thread owns one weight row: LDS.128 x 4 of its 64 packed bytes, nibble -> bf16 with
 //               ONE lop3 per pair ((w >> 4t) & 0x000F000F | 0x43004300 = the pair 128 + u), tcgen05.st of the
 //               A operand into TMEM (the 4x expanded weights never touch shared memory), then the fp32
 //               scale-accumulate (tcgen05.ld + FMA) of the group it converted one iteration earlier.
-//   warp 1      one thread issues tcgen05.mma.kind::f16, A from TMEM, B (= X tile) from shared memory, into a
+//   warps 2-3   one thread each (even / odd groups) issues tcgen05.mma.kind::f16, A from TMEM, B (= X tile) from shared memory, into a
 //               fresh fp32 TMEM accumulator per group (so the group scale is applied exactly, in fp32, after the
 //               contraction).  For MPAD <= 32 the offset of the code (q = u - 8 = (128 + u) - 136) is folded
 //               into the contraction: eight more MMAs with a constant A tile of -136 accumulate -136 * sum_k x
@@ -35,23 +35,26 @@ using namespace er;
 constexpr int kTileN = 128;                 // weight rows per tile
 constexpr int kWBytes = kTileN * 64;        // 8 KiB packed weights per group stage
 constexpr int kScaleBytes = kTileN * 2;     // 128 bf16 scales
-constexpr int kThreads = 320;               // TMA warp + MMA warp + 8 worker warps
+constexpr int kThreads = 384;               // 2 producer warps + 2 MMA warps + 8 worker warps
 constexpr int kMaxStages = 16;
 constexpr int kTmemCols = 512;
-constexpr int kTmemA = 0;                   // A operand: 2 buffers (one per worker set) x 64 columns
-constexpr int kTmemConst = 128;             // 8 columns of bf16 pairs (-136, -136)
-constexpr int kTmemD = 256;                 // accumulators: 2 buffers x MPAD columns
+constexpr int kTmemA = 0;                   // A operand: 4 buffers (2 per worker set) x 64 columns
+constexpr int kTmemD = 256;                 // accumulators: 4 buffers (2 per worker set) x MPAD columns
+constexpr int kTmemConst = 384;             // 8 columns of bf16 pairs (-136, -136); only used when MPAD <= 32
 constexpr int kSmemLimit = 227 * 1024;
 
-template <int MPAD>
+template <int MPAD, bool kConst>
 struct Cfg {
-  static constexpr bool kConstOffset = (MPAD <= 32);       // fold the -136 into the contraction
+  static_assert(!kConst || MPAD <= 32, "the constant tile sits behind four accumulators of <= 32 columns");
+  static constexpr bool kConstOffset = kConst;             // fold the -136 into the contraction
   static constexpr int kXBytes = MPAD * 128 * 2;           // two boxes of [MPAD x 64] bf16
   static constexpr int kStageBytes = ((kWBytes + kXBytes + kScaleBytes + 1023) / 1024) * 1024;
   static constexpr int kRedBytes = MPAD * kTileN * 4;      // odd-set accumulators handed to the even set
   static constexpr int kFixed = kRedBytes + 1024 /*align slack*/ + 512 /*barriers*/;
   static constexpr int kStagesRaw = (kSmemLimit - kFixed) / kStageBytes;
-  static constexpr int kStages = kStagesRaw > kMaxStages ? kMaxStages : kStagesRaw;
+  // even: each producer / worker set then cycles through its own half of the ring (an odd ring would let the
+  // even producer lap a stage that only the odd set's progress had released)
+  static constexpr int kStages = (kStagesRaw > kMaxStages ? kMaxStages : kStagesRaw) & ~1;
   static constexpr int kSmem = kStages * kStageBytes + kFixed;
   static constexpr uint32_t kTxBytes = kWBytes + kXBytes + kScaleBytes;
 };
@@ -71,7 +74,23 @@ struct GemmParams {
   float* partials;     // workspace + ER_GEMM_COUNTER_BYTES: [cta][2][MPAD][128]
   int* counters;       // workspace: one ticket per tile
   int dbg;             // debug/sweep flags (er_gemm_tuning key 2); 0 in production
+#ifdef ER_GEMM_TRACE
+  unsigned long long* trace;
+#endif
 };
+
+// Optional in-kernel timeline (development builds only, -DER_GEMM_TRACE): lane 0 of every warp of CTA 0 logs
+// (event id, clock) pairs.
+#ifdef ER_GEMM_TRACE
+#define ER_TR(id)                                                                                     \
+  do {                                                                                                \
+    if (p.trace && blockIdx.x == 0 && (threadIdx.x & 31) == 0 && tr_n < 500) {                        \
+      p.trace[((threadIdx.x >> 5) * 512 + tr_n++)] = ((unsigned long long)(id) << 48) | (clock64() & 0xFFFFFFFFFFFFull); \
+    }                                                                                                 \
+  } while (0)
+#else
+#define ER_TR(id) do {} while (0)
+#endif
 
 #define ER_TMEM_ST16(taddr, r, o)                                                                              \
   asm volatile(                                                                                                \
@@ -130,10 +149,10 @@ __device__ __forceinline__ int owner_of(long long units, int P, long long u) {
   return c;
 }
 
-template <int MPAD>
+template <int MPAD, bool kConst>
 __global__ void __launch_bounds__(kThreads, 1)
 w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
-  using C = Cfg<MPAD>;
+  using C = Cfg<MPAD, kConst>;
   constexpr int S = C::kStages;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -141,13 +160,17 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   uint64_t* bars = reinterpret_cast<uint64_t*>(smem + S * C::kStageBytes + C::kRedBytes);
   uint64_t* full = bars;                        // [S] TMA landed
   uint64_t* empty = bars + kMaxStages;          // [S] 4 worker warps + MMA commit released the stage
-  uint64_t* a_full = bars + 2 * kMaxStages;     // [2] A operand of a group written to TMEM (4 worker warps)
-  uint64_t* mma_done = a_full + 2;              // [2] MMAs of a group complete: D readable, A reusable
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(mma_done + 2);
+  uint64_t* a_full = bars + 2 * kMaxStages;     // [4] A operand of a group written to TMEM (4 worker warps)
+  uint64_t* mma_done = a_full + 4;              // [4] MMAs of a group complete: D readable, A reusable
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(mma_done + 4);
   int* last_flag = reinterpret_cast<int*>(tmem_slot + 1);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int P = gridDim.x, cta = blockIdx.x;
+#ifdef ER_GEMM_TRACE
+  int tr_n = 0;
+#endif
+  ER_TR(1);
   const int ug = p.unit_groups;
   const long long gb = range_begin(p.units, P, cta) * ug;        // first global group index of this CTA
   const long long ge = range_begin(p.units, P, cta + 1) * ug;
@@ -159,55 +182,70 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
       mbar_init(&full[s], 1);
       mbar_init(&empty[s], 5);
     }
-    for (int j = 0; j < 2; ++j) {
+    for (int j = 0; j < 4; ++j) {
       mbar_init(&a_full[j], 4);
       mbar_init(&mma_done[j], 1);
     }
     mbar_fence_init();
   }
-  if (warp == 1) tmem_alloc<kTmemCols>(tmem_slot);
+  if (warp == 2) tmem_alloc<kTmemCols>(tmem_slot);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = *tmem_slot;
+  ER_TR(2);
 
-  if (warp == 0) {
-    // ===================== TMA producer =====================
-    if (lane == 0) {
-      for (int it = 0; it < n_it; ++it) {
+  if (warp < 2) {
+    // ===================== producers: warp 0 feeds the even groups of the range, warp 1 the odd ones =========
+    // (one thread per parity: the issue loop of a single thread is latency-bound at ~10 cycles per instruction,
+    //  so it is kept free of divisions and split in two)
+    if (lane == 0 && warp < n_it) {
+      int it = warp;
+      const long long gi = gb + it;
+      int tile = (int)(gi / p.G), g = (int)(gi % p.G);
+      int tn = tile % p.ntiles, mc = tile / p.ntiles;
+      for (; it < n_it; it += 2) {
         const int s = it % S;
         mbar_wait(&empty[s], ((it / S) & 1) ^ 1);
-        const long long gi = gb + it;
-        const int tile = (int)(gi / p.G), g = (int)(gi % p.G);
-        const int n0 = (tile % p.ntiles) * kTileN, m0 = (tile / p.ntiles) * MPAD;
+        ER_TR(10);
         uint8_t* st = smem + s * C::kStageBytes;
         mbar_arrive_expect_tx(&full[s], C::kTxBytes);
         // ER_PACK_V2: the [128 rows x 128 k] block of (tile, g) is 8 KiB of contiguous, pre-swizzled bytes
-        bulk_load_1d(st, p.qweight + ((size_t)(tile % p.ntiles) * p.G + g) * kWBytes, kWBytes, &full[s], kEvictFirst);
-        tma_load_2d(st + kWBytes, &map_x, &full[s], g * 128, m0, kEvictLast);
-        tma_load_2d(st + kWBytes + MPAD * 128, &map_x, &full[s], g * 128 + 64, m0, kEvictLast);
-        bulk_load_1d(st + kWBytes + C::kXBytes, p.scales + ((size_t)g * p.N + n0) * 2, kScaleBytes, &full[s],
+        bulk_load_1d(st, p.qweight + ((size_t)tn * p.G + g) * kWBytes, kWBytes, &full[s], kEvictFirst);
+        tma_load_2d(st + kWBytes, &map_x, &full[s], g * 128, mc * MPAD, kEvictLast);
+        tma_load_2d(st + kWBytes + MPAD * 128, &map_x, &full[s], g * 128 + 64, mc * MPAD, kEvictLast);
+        bulk_load_1d(st + kWBytes + C::kXBytes, p.scales + ((size_t)g * p.N + tn * kTileN) * 2, kScaleBytes, &full[s],
                      kEvictFirst);
+        ER_TR(11);
+        g += 2;
+        while (g >= p.G) {
+          g -= p.G;
+          if (++tn == p.ntiles) { tn = 0; ++mc; }
+        }
       }
     }
-  } else if (warp == 1) {
-    // ===================== MMA issuer =====================
+  } else if (warp < 4) {
+    // ===================== MMA issuers: warp 2 for the even groups (worker set 0), warp 3 for the odd ones =====
     if (lane == 0) {
       constexpr uint32_t idesc = idesc_bf16_m128(MPAD);
-      for (int it = 0; it < n_it; ++it) {
-        const int s = it % S, j = it & 1;
+      const int set = warp - 2;
+      for (int it = set; it < n_it; it += 2) {
+        const int s = it % S, j = set * 2 + ((it >> 1) & 1);   // buffer: set, then the set's own parity
         mbar_wait(&full[s], (it / S) & 1);
-        mbar_wait(&a_full[j], (it >> 1) & 1);
+        ER_TR(20);
+        if (p.dbg & 64) { mbar_arrive(&empty[s]); continue; }
+        mbar_wait(&a_full[j], (it >> 2) & 1);
+        ER_TR(21);
         tc_fence_after();
         const uint32_t xbase = smem_u32(smem + s * C::kStageBytes + kWBytes);
         const uint32_t d_t = tmem + kTmemD + j * MPAD;
         const uint32_t a_t = tmem + kTmemA + j * 64;
         if (!(p.dbg & 1)) {
 #pragma unroll
-        for (int kk = 0; kk < 8; ++kk) {
-          const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
-          mma_ts_f16(d_t, a_t + kk * 8, bdesc, idesc, kk > 0 ? 1u : 0u);
-        }
+          for (int kk = 0; kk < 8; ++kk) {
+            const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
+            mma_ts_f16(d_t, a_t + kk * 8, bdesc, idesc, kk > 0 ? 1u : 0u);
+          }
         }
         if (C::kConstOffset && !(p.dbg & 2)) {
 #pragma unroll
@@ -216,17 +254,19 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
             mma_ts_f16(d_t, tmem + kTmemConst, bdesc, idesc, 1u);
           }
         }
+        ER_TR(22);
         tc_commit(&mma_done[j]);
         tc_commit(&empty[s]);
+        ER_TR(23);
       }
     }
   } else {
     // ===================== workers: dequant -> TMEM, scale-accumulate, output =====================
-    const int set = (warp - 2) >> 2;       // 0: even groups of the range, 1: odd groups
+    const int set = (warp - 4) >> 2;       // 0: even groups of the range, 1: odd groups
     const int q4 = warp & 3;               // TMEM lane quarter this warp may access
     const int row = q4 * 32 + lane;        // weight row inside the tile
     const uint32_t lane_addr = (uint32_t)(q4 * 32) << 16;
-    if (C::kConstOffset && set == 0) {     // constant A tile: bf16 pairs (-136, -136), written once
+    if (C::kConstOffset) {                 // constant A tile: bf16 pairs (-136, -136); both sets write the same values
       uint32_t c8[16];
 #pragma unroll
       for (int i = 0; i < 16; ++i) c8[i] = 0xC308C308u;
@@ -256,33 +296,44 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
       float sc_prev = 0.f;
 
       auto epilogue_group = [&](int it_done, float sc) {
-        mbar_wait(&mma_done[set], (it_done >> 1) & 1);
+        const int b = set * 2 + ((it_done >> 1) & 1);
+        if (p.dbg & 16) return;
+        ER_TR(35);
+        mbar_wait(&mma_done[b], (it_done >> 2) & 1);
+        ER_TR(36);
+        if (p.dbg & 8) return;
         tc_fence_after();
         uint32_t d[MPAD];
 #pragma unroll
-        for (int c = 0; c < MPAD; c += 16) ER_TMEM_LD16(tmem + lane_addr + kTmemD + set * MPAD + c, d, c);
+        for (int c = 0; c < MPAD; c += 16) ER_TMEM_LD16(tmem + lane_addr + kTmemD + b * MPAD + c, d, c);
         asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
         for (int m = 0; m < MPAD; ++m) acc[m] = fmaf(sc, __uint_as_float(d[m]), acc[m]);
+        ER_TR(37);
       };
 
       int my = it + ((it & 1) != set ? 1 : 0);
       for (; my < it_end; my += 2) {
         const int s = my % S;
+        ER_TR(30);
         mbar_wait(&full[s], (my / S) & 1);
+        ER_TR(31);
+        if (p.dbg & 64) { __syncwarp(); if (lane == 0) mbar_arrive(&empty[s]); continue; }
         const uint8_t* st = smem + s * C::kStageBytes;
         const uint8_t* wrow = st + row * 64;
         uint4 pk[4];
 #pragma unroll
         for (int c = 0; c < 4; ++c) pk[c] = *reinterpret_cast<const uint4*>(wrow + ((c ^ ((row >> 1) & 3)) << 4));
+        if (p.dbg & 32) { pk[1] = pk[0]; pk[2] = pk[0]; pk[3] = pk[0]; }
         const float sc =
             __bfloat162float(*reinterpret_cast<const __nv_bfloat16*>(st + kWBytes + C::kXBytes + row * 2));
-        if (pending && !(p.dbg & 8)) epilogue_group(my - 2, sc_prev);
         uint32_t a[64];
 #pragma unroll
         for (int c = 0; c < 4; ++c) dequant4<!C::kConstOffset>(pk[c], a, 16 * c);
-        // A[set] is free: the MMAs of this set's previous group were waited for in the epilogue above
-        const uint32_t a_t = tmem + lane_addr + kTmemA + set * 64;
+        // this A buffer was last read by the MMAs of group my - 4, waited for in the previous iteration's epilogue
+        const int b = set * 2 + ((my >> 1) & 1);
+        const uint32_t a_t = tmem + lane_addr + kTmemA + b * 64;
+        ER_TR(32);
         if (!(p.dbg & 4)) {
         ER_TMEM_ST16(a_t + 0, a, 0);
         ER_TMEM_ST16(a_t + 16, a, 16);
@@ -290,17 +341,22 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
         ER_TMEM_ST16(a_t + 48, a, 48);
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         } else { if (a[0] + a[17] + a[35] + a[63] == 0x12345u) *last_flag = 1; }
+        ER_TR(33);
         tc_fence_before();
         __syncwarp();
         if (lane == 0) {
           mbar_arrive(&empty[s]);   // every lane's shared-memory reads of this stage have been consumed
-          mbar_arrive(&a_full[set]);
+          mbar_arrive(&a_full[b]);
         }
+        ER_TR(34);
+        // scale-accumulate the group converted one iteration ago: its MMAs had this whole iteration to finish
+        if (pending) epilogue_group(my - 2, sc_prev);
         pending = true;
         sc_prev = sc;
       }
-      if (pending && !(p.dbg & 8)) epilogue_group(my - 2, sc_prev);
+      if (pending) epilogue_group(my - 2, sc_prev);
 
+      ER_TR(40);
       // ---- combine the two sets (odd -> shared memory -> even) ----
       if (set == 1) {
         if (seg > 0) named_bar_sync(2, 256);          // even set has finished reading the previous segment's red
@@ -327,7 +383,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
           named_bar_sync(3, 128);
           const long long u_first = ((long long)tile * p.G) / ug, u_last = ((long long)(tile + 1) * p.G - 1) / ug;
           const int c_lo = owner_of(p.units, P, u_first), c_hi = owner_of(p.units, P, u_last);
-          if (threadIdx.x == 64) {
+          if (threadIdx.x == 128) {
             const int old = atomicAdd(p.counters + tile, 1);
             const int last = (old == c_hi - c_lo);
             if (last) p.counters[tile] = 0;  // leave the counter zero for the next call
@@ -365,6 +421,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
           }
         }
       }
+      ER_TR(41);
       it = it_end;
       ++seg;
     }
@@ -373,7 +430,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
-  if (warp == 1) tmem_dealloc<kTmemCols>(tmem);
+  if (warp == 2) tmem_dealloc<kTmemCols>(tmem);
 }
 
 }  // namespace
@@ -413,7 +470,11 @@ bool make_map_2d(CUtensorMap* map, CUtensorMapDataType dt, const void* base, uin
   return r == CUDA_SUCCESS;
 }
 
+#ifdef ER_GEMM_TRACE
+unsigned long long* g_trace = nullptr;
+#endif
 int g_tune_dbg = 0;
+int g_tune_const = 0;      // 1: fold the -136 code offset into the contraction (MPAD <= 32)
 int g_tune_force_ctas = 0;  // > 0: use this many CTAs (tests / sweeps); 0 = one per SM
 
 struct Plan {
@@ -444,15 +505,15 @@ size_t workspace_for(int mpad) {
   return ER_GEMM_COUNTER_BYTES + (size_t)er::sm_count() * 2 * mpad * kTileN * sizeof(float);
 }
 
-template <int MPAD>
+template <int MPAD, bool kConst>
 int launch(const CUtensorMap& mx, const GemmParams& gp, const Plan& pl, cudaStream_t stream) {
   static bool attr_set = false;
   if (!attr_set) {
-    ER_CUDA_TRY(cudaFuncSetAttribute(w4a16_gemm_kernel<MPAD>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                     Cfg<MPAD>::kSmem));
+    ER_CUDA_TRY(cudaFuncSetAttribute(w4a16_gemm_kernel<MPAD, kConst>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     Cfg<MPAD, kConst>::kSmem));
     attr_set = true;
   }
-  w4a16_gemm_kernel<MPAD><<<pl.ctas, kThreads, Cfg<MPAD>::kSmem, stream>>>(mx, gp);
+  w4a16_gemm_kernel<MPAD, kConst><<<pl.ctas, kThreads, Cfg<MPAD, kConst>::kSmem, stream>>>(mx, gp);
   ER_CUDA_TRY(cudaGetLastError());
   return ER_OK;
 }
@@ -467,8 +528,13 @@ int er_gemm_tuning(int key, int value) {
   if (key == 0 && (value == 1 || value == 2)) return ER_OK;
   if (key == 1 && value >= 0) { g_tune_force_ctas = value; return ER_OK; }
   if (key == 2 && value >= 0) { g_tune_dbg = value; return ER_OK; }
+  if (key == 3 && (value == 0 || value == 1)) { g_tune_const = value; return ER_OK; }
   return ER_ERR_SHAPE;
 }
+
+#ifdef ER_GEMM_TRACE
+void er_gemm_set_trace(void* dev_ptr) { g_trace = reinterpret_cast<unsigned long long*>(dev_ptr); }
+#endif
 
 size_t er_gemm_workspace_bytes(int64_t M, int64_t N, int64_t K) {
   if (M < 1 || N < kTileN || N % kTileN != 0 || K < ER_GROUP || K % ER_GROUP != 0) return 0;
@@ -510,15 +576,18 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
   gp.M = (int)M; gp.N = (int)N; gp.K = (int)K;
   gp.G = pl.G; gp.ntiles = pl.ntiles; gp.tiles = pl.tiles; gp.unit_groups = pl.unit_groups; gp.units = pl.units;
   gp.dbg = g_tune_dbg;
+#ifdef ER_GEMM_TRACE
+  gp.trace = g_trace;
+#endif
   gp.qweight = reinterpret_cast<const uint8_t*>(qweight);
   gp.scales = reinterpret_cast<const uint8_t*>(scales);
   gp.y_f32 = (y_dtype == ER_F32); gp.ldy = ldy_elems; gp.y = y;
   gp.counters = reinterpret_cast<int*>(workspace);
   gp.partials = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + ER_GEMM_COUNTER_BYTES);
   cudaStream_t s = (cudaStream_t)stream;
-  if (pl.mpad == 16) return launch<16>(mx, gp, pl, s);
-  if (pl.mpad == 32) return launch<32>(mx, gp, pl, s);
-  return launch<64>(mx, gp, pl, s);
+  if (pl.mpad == 16) return g_tune_const ? launch<16, true>(mx, gp, pl, s) : launch<16, false>(mx, gp, pl, s);
+  if (pl.mpad == 32) return g_tune_const ? launch<32, true>(mx, gp, pl, s) : launch<32, false>(mx, gp, pl, s);
+  return launch<64, false>(mx, gp, pl, s);
 }
 
 }  // extern "C"
