@@ -79,6 +79,20 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
       : "memory");
 }
 
+// The same two on a shared-window address that is already in a register.
+__device__ __forceinline__ void mbar_arrive_addr(uint32_t a) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(a) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_addr(uint32_t a, uint32_t parity) {
+  asm volatile(
+      "{\n\t.reg .pred P1;\n\t"
+      "ER_WAITA_%=:\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+      "@!P1 bra ER_WAITA_%=;\n\t}\n" ::"r"(a),
+      "r"(parity)
+      : "memory");
+}
+
 // Same, as a tight poll (mbarrier.test_wait never suspends): for the one polling warp of a role, where the
 // wake-up delay of try_wait would sit on the critical path of the buffer ring.
 __device__ __forceinline__ void mbar_spin(uint64_t* bar, uint32_t parity) {

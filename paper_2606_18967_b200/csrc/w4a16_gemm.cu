@@ -2,10 +2,12 @@
 // (dense projections are ~90 % of tail decode latency and weight loading dominates at
 // small batch; L175: W4A16 weight-only kernel; L467: "on-the-fly dequantization and kernel-level overhead").
 //
-// sm_100a design, third version.  The first two were bound by one long
-// wait -> convert -> MMA -> read-back chain per warp and by single-thread issue loops whose TMA / MMA
-// operands the compiler could not prove warp-uniform (profiles/r01_*): here every role is its own warp(s),
-// the chains only meet at mbarriers, and the issuing warps run warp-uniform code with one elected lane.
+// sm_100a design, fourth version.  What the earlier ones taught
+// (profiles/r01_*): TMA / MMA issue must be warp-uniform code with one elected lane (otherwise the
+// compiler wraps every instruction in a per-lane loop); a closed ring of few TMEM buffers between separate
+// converter / MMA / read-back roles is bound by the round-trip latency of its mbarriers; and the nibble ->
+// bf16 conversion (7 logic-pipe operations per packed word, the logic pipe runs at half rate) is the
+// largest fixed cost, about 224 cycles per 128-k group and SM sub-partition, so it must never wait.
 //
 //   persistent   one CTA per SM; the (tile, 128-k group) units of the whole problem are dealt out as ONE
 //                contiguous range per CTA ("stream-K"): every CTA streams the same number of bytes.
@@ -15,18 +17,17 @@
 //                scales and two SWIZZLE_128B TMA boxes of X [MPAD x 64 k], into a ring of up to 16 stages.
 //   warp 1       MMA issuer: tcgen05.mma.kind::f16, A (weights) from TENSOR MEMORY, B (= X tile) from shared
 //                memory, a fresh fp32 TMEM accumulator per group so the group scale is applied exactly.
-//   warps 4-19   converters, two sets of 8 (even / odd groups).  A thread owns HALF a weight row of the
-//                group: 2 x LDS.128, nibble -> 16-bit float with the magic-number trick, tcgen05.st into the
-//                A buffer (the 4x expanded weights never touch shared memory).
-//   warps 20-27  scale-accumulate: tcgen05.ld of the group's accumulator, acc += scale * d in fp32 registers,
-//                and the output: a tile wholly owned by one CTA is stored directly, otherwise fp32 partials go
-//                to the workspace and the last CTA of the tile (ticket counter) adds them in ascending CTA
-//                order.  Deterministic, no float atomics.
-//   TMEM         4 A buffers (64 columns each) and 8 (MPAD = 64: 4) accumulators cycle independently: an A
-//                buffer is refilled once the MMAs that read it completed, an accumulator once it was drained.
-//   barriers     full[stage] (TMA landed), done[stage] (ONE tcgen05.commit per group: accumulator readable, A
-//                buffer and shared-memory stage reusable), a_full[A buffer], d_free[accumulator].  One warp per
-//                role polls (tight test_wait) and releases its peers through a named barrier.
+//   warps 4-27   three self-paced worker sets of 8 warps; set j owns the groups j, j+3, ... of the CTA's
+//                range, one A buffer and one accumulator in TMEM.  A thread owns HALF a weight row of the
+//                group.  Per group: 2 x LDS.128, nibble -> bf16 ((w >> 4t) & 0x000F000F | 0x43004300 = the
+//                pair 128 + u, one packed fma removes the 136), then the scale-accumulate of the set's
+//                PREVIOUS group (tcgen05.ld + fma: its MMAs had the whole conversion to finish), then
+//                tcgen05.st of the new A operand (the 4x expanded weights never touch shared memory) and
+//                an arrival on the set's a_full barrier.  The three sets interleave on the logic pipe.
+//   output       at the end of a tile segment sets 1-2 hand their partial sums to set 0 through shared memory;
+//                a tile wholly owned by one CTA is stored directly, otherwise fp32 partials go to the workspace
+//                and the last CTA of the tile (ticket counter) adds them in ascending CTA order.
+//                Deterministic, no float atomics.
 #include <cuda.h>
 #include "er_common.cuh"
 
@@ -37,28 +38,33 @@ using namespace er;
 constexpr int kTileN = 128;                 // weight rows per tile
 constexpr int kWBytes = kTileN * 64;        // 8 KiB packed weights per group stage
 constexpr int kScaleBytes = kTileN * 2;     // 128 bf16 scales
-constexpr int kCvtWarp0 = 4, kCvtWarps = 16;    // converter warps 4..19
-constexpr int kEpiWarp0 = 20, kEpiWarps = 8;    // scale-accumulate warps 20..27
-constexpr int kThreads = (kEpiWarp0 + kEpiWarps) * 32;   // 896
+constexpr int kSets = 3;                    // worker sets
+constexpr int kSetWarp0 = 4;                // worker warps 4..27, 8 per set
+constexpr int kSetThreads = 256;
+constexpr int kThreads = (kSetWarp0 + kSets * 8) * 32;   // 896
 constexpr int kMaxStages = 16;
-constexpr int kNA = 4;                      // A-operand buffers in TMEM
 constexpr int kTmemCols = 512;
-constexpr int kTmemA = 0;                   // A operand: kNA buffers x 64 columns
-constexpr int kTmemD = 256;                 // accumulators: kND buffers x MPAD columns
+constexpr int kTmemA = 0;                   // A operand: kBuf 64-column buffers per set
 constexpr int kSmemLimit = 227 * 1024;
 
 template <int MPAD>
 struct Cfg {
   static constexpr int kXBytes = MPAD * 128 * 2;           // two boxes of [MPAD x 64] bf16
   static constexpr int kStageBytes = ((kWBytes + kXBytes + kScaleBytes + 1023) / 1024) * 1024;
-  static constexpr int kND = MPAD <= 32 ? 8 : 4;           // accumulator buffers in TMEM (kND * MPAD <= 256 columns)
-  static constexpr int kScBufBytes = kMaxStages * kTileN * 4;   // fp32 scales of the groups in flight, by stage
-  static constexpr int kFixed = kScBufBytes + 1024 /*align slack*/ + 512 /*barriers*/;
+  static constexpr int kRedBytes = (kSets - 1) * MPAD * kTileN * 4;   // partial sums of sets 1.. handed to set 0
+  static constexpr int kFixed = kRedBytes + 1024 /*align slack*/ + 512 /*barriers*/;
   static constexpr int kStagesRaw = (kSmemLimit - kFixed) / kStageBytes;
   static constexpr int kStages = kStagesRaw > kMaxStages ? kMaxStages : kStagesRaw;
   static constexpr int kSmem = kStages * kStageBytes + kFixed;
   static constexpr uint32_t kTxBytes = kWBytes + kXBytes + kScaleBytes;
-  static constexpr int kCW = MPAD / 2;                     // accumulator columns per scale-accumulate warp
+  static constexpr int kCW = MPAD / 2;                     // accumulator columns per thread (half of the batch rows)
+  static constexpr bool kEpiFirst = (MPAD > 32);           // register pressure: read back before converting
+  // TMEM: every set owns kBuf (A operand, accumulator) pairs.  Two pairs (M <= 16, where the columns allow it)
+  // let a set convert group i + 1 while the MMAs of group i are still in flight.
+  static constexpr int kBuf = (MPAD == 16) ? 2 : 1;
+  static constexpr int kTmemConst = kSets * kBuf * 64;     // per set 8 columns of bf16 pairs (-136, -136): the constant A tile
+  static constexpr int kTmemD = (kTmemConst + 8 * kSets + MPAD - 1) / MPAD * MPAD;   // accumulators, MPAD columns each
+  static_assert(kTmemD + kSets * kBuf * MPAD <= kTmemCols, "TMEM columns");
 };
 
 struct GemmParams {
@@ -127,15 +133,14 @@ __device__ __forceinline__ uint32_t lop3_and_or(uint32_t a, uint32_t mask, uint3
 }
 
 // One packed word (8 codes; nibble positions (t, t + 4) hold the consecutive pair k = 2t, 2t + 1) -> 4 registers
-// of bf16 pairs holding q = u - 8 exactly: (w >> 4t) & 0x000F000F | 0x43004300 is the pair (128 + u, 128 + u'),
-// one packed fma (x * 1 - 136, on the FMA pipe) removes the offset.  7 logic-pipe + 4 FMA-pipe ops per word.
+// of bf16 pairs (128 + u, 128 + u'): (w >> 4t) & 0x000F000F | 0x43004300, i.e. 3 shifts + 4 lop3 per word, all
+// on the half-rate logic pipe.  The stored nibble is u = q + 8, so the A operand is q + 136; the -136 is NOT
+// removed here (one packed fma per pair would cost as many issue cycles again) but folded into the
+// contraction: eight more MMAs per group with a constant A tile of -136 add -136 * sum_k x to the accumulator.
 // (An fp16 A operand would need 5 logic ops, but tcgen05.mma.kind::f16 faults on fp16 A x bf16 B.)
 __device__ __forceinline__ void dequant_word(uint32_t w, uint32_t* a) {
 #pragma unroll
-  for (int t = 0; t < 4; ++t) {
-    const uint32_t v = lop3_and_or(w >> (4 * t), 0x000F000Fu, 0x43004300u);
-    asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(a[t]) : "r"(v), "r"(0x3F803F80u), "r"(0xC308C308u));
-  }
+  for (int t = 0; t < 4; ++t) a[t] = lop3_and_or(w >> (4 * t), 0x000F000Fu, 0x43004300u);
 }
 
 __device__ __forceinline__ uint4 lds128(uint32_t saddr) {
@@ -169,22 +174,23 @@ __device__ __forceinline__ int owner_of(long long units, int P, long long u) {
   return c;
 }
 
+__device__ __forceinline__ void named_bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+
 template <int MPAD>
 __global__ void __launch_bounds__(kThreads, 1)
 w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
   using C = Cfg<MPAD>;
   constexpr int S = C::kStages;
-  constexpr int ND = C::kND;
+  constexpr int kBuf = C::kBuf;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
-  float* sc_buf = reinterpret_cast<float*>(smem + S * C::kStageBytes);          // [S][128]
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + S * C::kStageBytes + C::kScBufBytes);
-  uint64_t* full = bars;                        // [S]   TMA landed
-  uint64_t* done = bars + kMaxStages;           // [S]   the group's MMAs have completed: accumulator readable,
-                                                //       A buffer and shared-memory stage reusable
-  uint64_t* a_full = bars + 2 * kMaxStages;     // [kNA] A operand (and scales) of a group written
-  uint64_t* d_free = a_full + kNA;              // [ND]  accumulator drained
-  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(d_free + 8);
+  float* red = reinterpret_cast<float*>(smem + S * C::kStageBytes);             // [kSets-1][MPAD][128]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + S * C::kStageBytes + C::kRedBytes);
+  uint64_t* full = bars;                        // [S]     TMA landed
+  uint64_t* empty = bars + kMaxStages;          // [S]     the group's MMAs completed: the stage may be refilled
+  uint64_t* a_full = bars + 2 * kMaxStages;     // [kSets][kBuf] the A operand is written, its accumulator drained
+  uint64_t* done = a_full + 8;                  // [kSets][kBuf] the MMAs completed: accumulator readable, A free
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(done + 8);
   int* last_flag = reinterpret_cast<int*>(tmem_slot + 1);
 
   const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);   // provably warp-uniform
@@ -202,10 +208,12 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   if (warp == 0) {
     if (lane < S) {
       mbar_init(&full[lane], 1);
+      mbar_init(&empty[lane], 1);
+    }
+    if (lane < kSets * C::kBuf) {
+      mbar_init(&a_full[lane], 8);
       mbar_init(&done[lane], 1);
     }
-    if (lane < kNA) mbar_init(&a_full[lane], 8);
-    if (lane < ND) mbar_init(&d_free[lane], kEpiWarps);
     mbar_fence_init();
     if (lane == 0) tma_prefetch_desc(&map_x);
   }
@@ -223,7 +231,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
     int s = 0;
     uint32_t ph = 0;
     for (int it = 0; it < n_it; ++it) {
-      mbar_spin(&done[s], ph ^ 1);      // the stage's previous group (it - S) has been contracted
+      mbar_wait(&empty[s], ph ^ 1);      // the stage's previous group (it - S) has been contracted
       ER_TR(1);
       if (elect_one()) {
         uint8_t* st = smem + s * C::kStageBytes;
@@ -243,209 +251,253 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
       }
       if (++s == S) { s = 0; ph ^= 1; }
     }
-  } else if (warp == 1) {
-    // ===================== MMA issuer (warp-uniform; one elected lane issues) =====================
+  } else if (warp <= kBuf) {
+    // ===================== MMA issuers (warp-uniform; one elected lane issues) =====================
+    // With two buffers per set, warp 1 takes the even groups of the range and warp 2 the odd ones (they sit on
+    // different SM sub-partitions, whose issue slots the worker warps keep busy: one issuer alone is too slow).
+    // A given (set, buffer) pair is then always served by the same issuer, which therefore sees every phase
+    // of its a_full barrier; with one buffer per set that would not hold, so a single warp issues everything.
     constexpr uint32_t idesc = idesc_bf16_m128(MPAD);
-    int s = 0;
-    for (int it = 0; it < n_it; ++it) {
-      const int ia = it & (kNA - 1), id = it & (ND - 1);
+    int s = warp - 1;
+    uint32_t ph = 0;                     // parity of full[s] (streaming-only mode)
+    for (int it = warp - 1; it < n_it; it += kBuf) {
       if (p.dbg & 64) {
-        mbar_spin(&full[s], (it / S) & 1);
-        if (elect_one()) mbar_arrive(&done[s]);
+        mbar_wait(&full[s], ph);
+        if (elect_one()) mbar_arrive(&empty[s]);
       } else {
-        mbar_spin(&a_full[ia], (it / kNA) & 1);          // implies full[s]: the converters waited for it
-        mbar_spin(&d_free[id], ((it / ND) & 1) ^ 1);     // accumulator of group it - ND drained
+        const int i = it / kSets, set = it - i * kSets;   // the set's i-th group
+        const int bi = set * kBuf + (i % kBuf);
+        mbar_wait(&a_full[bi], (i / kBuf) & 1);            // implies full[s] (the set waited for it)
         ER_TR(1);
         tc_fence_after();
         if (elect_one()) {
           const uint32_t xbase = smem_u32(smem + s * C::kStageBytes + kWBytes);
-          const uint32_t d_t = tmem + kTmemD + id * MPAD;
-          const uint32_t a_t = tmem + kTmemA + ia * 64;
+          const uint32_t d_t = tmem + C::kTmemD + bi * MPAD;
+          const uint32_t a_t = tmem + kTmemA + bi * 64;
 #pragma unroll
           for (int kk = 0; kk < 8; ++kk) {
             const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
-            mma_ts_f16((p.dbg & 256) ? (tmem + kTmemD + 128 + kk * 16) : d_t, a_t + kk * 8, bdesc, idesc, kk > 0 ? 1u : 0u);
+            mma_ts_f16(d_t, a_t + kk * 8, bdesc, idesc, kk > 0 ? 1u : 0u);
           }
-          tc_commit(&done[s]);
+#pragma unroll
+          for (int kk = 0; kk < 8; ++kk) {   // - 136 * sum_k x[m][k]: the offset of the stored nibble
+            const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
+            mma_ts_f16(d_t, tmem + C::kTmemConst + set * 8, bdesc, idesc, 1u);
+          }
+          tc_commit(&done[bi]);
+          tc_commit(&empty[s]);
         }
       }
       __syncwarp();
       ER_TR(2);
-      if (++s == S) s = 0;
+      s += kBuf;
+      if (s >= S) { s -= S; ph ^= 1; }
     }
-  } else if (warp >= kCvtWarp0 && warp < kCvtWarp0 + kCvtWarps) {
-    // ===================== converters: packed int4 -> bf16 A operand in TMEM =====================
-    const int dw = warp - kCvtWarp0;
-    const int set = dw >> 3;               // 0: even groups of the range, 1: odd groups
-    const int half = (dw >> 2) & 1;        // which 64 k of the group's 128 this thread converts
+  } else if (warp >= kSetWarp0) {
+    // ===================== worker sets: convert, scale-accumulate, output =====================
+    constexpr int CW = C::kCW;
+    const int dw = warp - kSetWarp0;
+    const int set = dw >> 3;               // groups set, set + 3, ... of the CTA's range
+    const int half = (dw >> 2) & 1;        // which 64 k of a group this thread converts / which half of the batch rows
     const int q4 = warp & 3;               // TMEM lane quarter this warp may access
     const int row = q4 * 32 + lane;        // weight row inside the tile
     const uint32_t lane_addr = (uint32_t)(q4 * 32) << 16;
     const int sw = (row >> 1) & 3;
-    const uint32_t smem_s = smem_u32(smem);
-    const uint32_t row_off0 = row * 64 + (((2 * half) ^ sw) << 4), row_off1 = row * 64 + (((2 * half + 1) ^ sw) << 4);
-    const uint32_t sc_s = smem_u32(sc_buf) + row * 4;
-    const bool poller = ((dw & 7) == 0);   // one warp of the set polls the mbarriers, a named barrier releases the
-                                           // other seven (a blocked bar.sync costs no issue slots, a poll loop does)
-    int s = set;                           // stage of group `it`
-    uint32_t ph = 0;
-    int sp = set + S - kNA;                // stage of group it - kNA (whose MMAs read this A buffer last)
-    uint32_t php = 1;                      // ... and the parity of that use; starts "one lap behind"
-    if (sp >= S) { sp -= S; php = 0; }
-    for (int it = set; it < n_it; it += 2) {
-      const int ia = it & (kNA - 1);
-      ER_TR(4);
-      if (poller) {
-        mbar_spin(&full[s], ph);
-        if (it >= kNA && !(p.dbg & 64)) mbar_spin(&done[sp], php);
-      }
-      named_bar_sync(1 + set, 256);
-      ER_TR(1);
-      if (p.dbg & 64) {
-        // streaming-only mode: nothing is converted
-      } else {
-        tc_fence_after();
-        const uint32_t st = smem_s + s * C::kStageBytes;
-        const uint4 pk0 = lds128(st + row_off0);
-        const uint4 pk1 = lds128(st + row_off1);
-        uint32_t sc16 = 0;
-        if (half == 0) sc16 = lds_u16(st + kWBytes + C::kXBytes + row * 2);
-        uint32_t a[32];
-        dequant_word(pk0.x, a + 0);
-        dequant_word(pk0.y, a + 4);
-        dequant_word(pk0.z, a + 8);
-        dequant_word(pk0.w, a + 12);
-        dequant_word(pk1.x, a + 16);
-        dequant_word(pk1.y, a + 20);
-        dequant_word(pk1.z, a + 24);
-        dequant_word(pk1.w, a + 28);
-        ER_TR(2);
-        const uint32_t a_t = tmem + lane_addr + kTmemA + ia * 64 + half * 32;
-        ER_TMEM_ST16(a_t + 0, a, 0);
-        ER_TMEM_ST16(a_t + 16, a, 16);
-        if (half == 0) sts_f32(sc_s + s * (kTileN * 4), __uint_as_float(sc16 << 16));
-        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&a_full[ia]);
-      }
-      ER_TR(3);
-      s += 2;
-      if (s >= S) { s -= S; ph ^= 1; }
-      sp += 2;
-      if (sp >= S) { sp -= S; php ^= 1; }
+    // loop invariants, pinned in registers (otherwise the compiler rematerialises the shared-window arithmetic
+    // in every iteration)
+    uint32_t w_addr0, w_addr1, sc_addr;
+    asm volatile("mov.u32 %0, %1;" : "=r"(w_addr0) : "r"(smem_u32(smem) + row * 64 + (((2 * half) ^ sw) << 4)));
+    asm volatile("mov.u32 %0, %1;" : "=r"(w_addr1) : "r"(smem_u32(smem) + row * 64 + (((2 * half + 1) ^ sw) << 4)));
+    asm volatile("mov.u32 %0, %1;" : "=r"(sc_addr) : "r"(smem_u32(smem) + kWBytes + C::kXBytes + row * 2));
+    uint32_t full_addr, done_addr, afull_addr;
+    asm volatile("mov.u32 %0, %1;" : "=r"(full_addr) : "r"(smem_u32(full)));
+    asm volatile("mov.u32 %0, %1;" : "=r"(done_addr) : "r"(smem_u32(&done[set * kBuf])));
+    asm volatile("mov.u32 %0, %1;" : "=r"(afull_addr) : "r"(smem_u32(&a_full[set * kBuf])));
+    const bool poller = ((dw & 7) == 0);   // one warp of the set polls `full`, a named barrier releases the other
+                                           // seven (a blocked bar.sync costs no issue slots, a poll loop does)
+    const bool leader = (threadIdx.x == kSetWarp0 * 32);
+    uint32_t a_t, d_t;
+    asm volatile("mov.u32 %0, %1;" : "=r"(a_t) : "r"(tmem + lane_addr + kTmemA + set * kBuf * 64 + half * 32));
+    asm volatile("mov.u32 %0, %1;" : "=r"(d_t) : "r"(tmem + lane_addr + C::kTmemD + set * kBuf * MPAD + half * CW));
+    const int bar_id = 1 + set;
+
+    if (half == 0) {                       // the set's constant A tile (-136, -136), one lane quarter per warp; ordered
+                                           // before the set's first MMA by its first a_full arrival
+      const uint32_t c = 0xC308C308u;
+      asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1};" ::"r"(
+                       tmem + lane_addr + C::kTmemConst + set * 8), "r"(c) : "memory");
+      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+      tc_fence_before();
     }
-  } else if (warp >= kEpiWarp0) {
-    // ===================== scale-accumulate + output =====================
-    constexpr int CW = C::kCW;
-    constexpr int kEpiThreads = kEpiWarps * 32;
-    const int ew = warp - kEpiWarp0;
-    const int ch = ew >> 2;                // which half of the accumulator columns (batch rows m)
-    const int q4 = warp & 3;
-    const int row = q4 * 32 + lane;
-    const uint32_t lane_addr = (uint32_t)(q4 * 32) << 16;
-    const bool leader = (threadIdx.x == kEpiWarp0 * 32);
-    const uint32_t sc_s = smem_u32(sc_buf) + row * 4;
+
     float acc[CW];
-    int it = 0;
-    int s = 0;
-    uint32_t ph = 0;
-    while (it < n_it && !(p.dbg & 64)) {
+    float sc_old = 0.f, sc_new = 0.f;      // scales of the (up to kBuf) groups whose MMAs are in flight
+    int npend = 0;                         // how many
+    uint32_t pd = 0;                       // bit b: parity of done[set][b] for its next read-back
+    int wbuf = 0, rbuf = 0;                // buffer the next group is written to / read back from
+    int my = set;                          // this set's next group (index into the CTA's range)
+    int s = set % S;                       // its stage ...
+    uint32_t ph = 0;                       // ... and the parity of full[s]
+    int it = 0, seg = 0;
+
+    // scale-accumulate of the set's pending group: acc += scale * (sum over its 128 k of x * q)
+    auto read_back = [&]() {
+      if (poller) mbar_wait_addr(done_addr + rbuf * 8, (pd >> rbuf) & 1);
+      named_bar_sync(bar_id, kSetThreads);
+      pd ^= 1u << rbuf;
+      tc_fence_after();
+      uint32_t d[CW];
+      const uint32_t dt = d_t + rbuf * MPAD;
+      if constexpr (CW == 8) {
+        ER_TMEM_LD8(dt, d, 0);
+      } else {
+#pragma unroll
+        for (int c = 0; c < CW; c += 16) ER_TMEM_LD16(dt + c, d, c);
+      }
+      asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+      for (int m = 0; m < CW; ++m) acc[m] = fmaf(sc_old, __uint_as_float(d[m]), acc[m]);
+      sc_old = sc_new;
+      --npend;
+      if (kBuf == 2) rbuf ^= 1;
+    };
+
+    while (it < n_it) {
       // ---- segment = the part of one tile inside this CTA's range ----
       const long long gi0 = gb + it;
       const int tile = (int)(gi0 / p.G), g_lo = (int)(gi0 % p.G);
       const int seg_len = min(p.G - g_lo, n_it - it);
       const int it_end = it + seg_len;
+      const bool last_seg = (it_end == n_it);
 #pragma unroll
       for (int m = 0; m < CW; ++m) acc[m] = 0.f;
-      for (int i = it; i < it_end; ++i) {
-        const int id = i & (ND - 1);
+      for (; my < it_end; my += kSets) {
         ER_TR(4);
-        if (ew == 0) mbar_spin(&done[s], ph);
-        named_bar_sync(4, kEpiThreads);
-        tc_fence_after();
+        if (poller) mbar_wait_addr(full_addr + s * 8, ph);
+        named_bar_sync(bar_id, kSetThreads);
         ER_TR(1);
-        uint32_t d[CW];
-        const uint32_t d_t = tmem + lane_addr + kTmemD + id * MPAD + ch * CW;
-        if constexpr (CW == 8) {
-          ER_TMEM_LD8(d_t, d, 0);
-        } else {
-#pragma unroll
-          for (int c = 0; c < CW; c += 16) ER_TMEM_LD16(d_t + c, d, c);
+        if (!(p.dbg & 64)) {
+          const uint32_t st = s * C::kStageBytes;
+          if (C::kEpiFirst && npend == kBuf) read_back();
+          const uint4 pk0 = lds128(st + w_addr0);
+          const uint4 pk1 = lds128(st + w_addr1);
+          const uint32_t sc16 = lds_u16(st + sc_addr);
+          uint32_t a[32];
+          dequant_word(pk0.x, a + 0);
+          dequant_word(pk0.y, a + 4);
+          dequant_word(pk0.z, a + 8);
+          dequant_word(pk0.w, a + 12);
+          dequant_word(pk1.x, a + 16);
+          dequant_word(pk1.y, a + 20);
+          dequant_word(pk1.z, a + 24);
+          dequant_word(pk1.w, a + 28);
+          ER_TR(2);
+          // the set's previous group: its MMAs had this whole conversion to finish; after this the A buffer
+          // (read by those MMAs) and the accumulator are free again
+          if (!C::kEpiFirst && npend == kBuf) read_back();
+          ER_TR(3);
+          ER_TMEM_ST16(a_t + wbuf * 64 + 0, a, 0);
+          ER_TMEM_ST16(a_t + wbuf * 64 + 16, a, 16);
+          asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive_addr(afull_addr + wbuf * 8);
+          if (npend == 0) sc_old = __uint_as_float(sc16 << 16);
+          else sc_new = __uint_as_float(sc16 << 16);
+          ++npend;
+          if (kBuf == 2) wbuf ^= 1;
         }
-        const float sc = lds_f32(sc_s + s * (kTileN * 4));
-        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
-        tc_fence_before();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&d_free[id]);
-#pragma unroll
-        for (int m = 0; m < CW; ++m) acc[m] = fmaf(sc, __uint_as_float(d[m]), acc[m]);
-        ER_TR(2);
-        if (++s == S) { s = 0; ph ^= 1; }
+        ER_TR(5);
+        s += kSets;
+        if (s >= S) { s -= S; ph ^= 1; }
       }
+      while (npend > 0) read_back();
+      ER_TR(6);
 
-      // ---- output: direct store, or partial + last-arriver reduction in ascending CTA order ----
-      const int n0 = (tile % p.ntiles) * kTileN, m0 = (tile / p.ntiles) * MPAD + ch * CW;
-      const int mvalid = min(CW, p.M - m0);     // may be <= 0: nothing of this half is a real batch row
-      const int n = n0 + row;
-      bool store = true;
-      if (seg_len != p.G) {
-        float* mine = p.partials + ((size_t)cta * 2 + (it == 0 ? 0 : 1)) * (MPAD * kTileN) + ch * CW * kTileN;
+      // ---- combine the three sets' partial sums in a fixed order (set 0 + set 1 + set 2), in set 0 ----
+      if (p.dbg & 64) {
+        it = it_end;
+        ++seg;
+        continue;
+      }
+      if (set != 0) {
+        if (seg > 0) named_bar_sync(5, kThreads - kSetWarp0 * 32);   // set 0 has read the previous segment's `red`
+        float* mine = red + ((set - 1) * MPAD + half * CW) * kTileN + row;
 #pragma unroll
-        for (int m = 0; m < CW; ++m)
-          if (m < mvalid) __stcg(mine + m * kTileN + row, acc[m]);
-        __threadfence();
-        named_bar_sync(3, kEpiThreads);
-        const long long u_first = ((long long)tile * p.G) / ug, u_last = ((long long)(tile + 1) * p.G - 1) / ug;
-        const int c_lo = owner_of(p.units, P, u_first), c_hi = owner_of(p.units, P, u_last);
-        if (leader) {
-          const int old = atomicAdd(p.counters + tile, 1);
-          const int last = (old == c_hi - c_lo);
-          if (last) p.counters[tile] = 0;  // leave the counter zero for the next call
-          *last_flag = last;
+        for (int m = 0; m < CW; ++m) mine[m * kTileN] = acc[m];
+        named_bar_arrive(6, kThreads - kSetWarp0 * 32);
+      } else {
+        named_bar_sync(6, kThreads - kSetWarp0 * 32);
+#pragma unroll
+        for (int j = 0; j < kSets - 1; ++j) {
+          const float* theirs = red + (j * MPAD + half * CW) * kTileN + row;
+#pragma unroll
+          for (int m = 0; m < CW; ++m) acc[m] += theirs[m * kTileN];
         }
-        named_bar_sync(3, kEpiThreads);
-        store = (*last_flag != 0);
-        if (store) {
-          __threadfence();
+        if (!last_seg) named_bar_arrive(5, kThreads - kSetWarp0 * 32);
+
+        // ---- output: direct store, or partial + last-arriver reduction in ascending CTA order ----
+        const int n0 = (tile % p.ntiles) * kTileN, m0 = (tile / p.ntiles) * MPAD + half * CW;
+        const int mvalid = min(CW, p.M - m0);     // may be <= 0: nothing of this half is a real batch row
+        const int n = n0 + row;
+        bool store = true;
+        if (seg_len != p.G) {
+          float* mine = p.partials + ((size_t)cta * 2 + (it == 0 ? 0 : 1)) * (MPAD * kTileN) + half * CW * kTileN;
 #pragma unroll
-          for (int m = 0; m < CW; ++m) acc[m] = 0.f;
-          for (int c = c_lo; c <= c_hi; ++c) {
-            // CTA c's piece of this tile is its first segment iff its range starts inside the tile
-            const long long cb = range_begin(p.units, P, c) * ug;
-            const int which = (cb >= (long long)tile * p.G) ? 0 : 1;
-            const float* src = p.partials + ((size_t)c * 2 + which) * (MPAD * kTileN) + ch * CW * kTileN;
+          for (int m = 0; m < CW; ++m)
+            if (m < mvalid) __stcg(mine + m * kTileN + row, acc[m]);
+          __threadfence();
+          named_bar_sync(7, kSetThreads);
+          const long long u_first = ((long long)tile * p.G) / ug, u_last = ((long long)(tile + 1) * p.G - 1) / ug;
+          const int c_lo = owner_of(p.units, P, u_first), c_hi = owner_of(p.units, P, u_last);
+          if (leader) {
+            const int old = atomicAdd(p.counters + tile, 1);
+            const int last = (old == c_hi - c_lo);
+            if (last) p.counters[tile] = 0;  // leave the counter zero for the next call
+            *last_flag = last;
+          }
+          named_bar_sync(7, kSetThreads);
+          store = (*last_flag != 0);
+          if (store) {
+            __threadfence();
+#pragma unroll
+            for (int m = 0; m < CW; ++m) acc[m] = 0.f;
+            for (int c = c_lo; c <= c_hi; ++c) {
+              // CTA c's piece of this tile is its first segment iff its range starts inside the tile
+              const long long cb = range_begin(p.units, P, c) * ug;
+              const int which = (cb >= (long long)tile * p.G) ? 0 : 1;
+              const float* src = p.partials + ((size_t)c * 2 + which) * (MPAD * kTileN) + half * CW * kTileN;
+#pragma unroll
+              for (int m = 0; m < CW; ++m)
+                if (m < mvalid) acc[m] += __ldcg(src + m * kTileN + row);
+            }
+          }
+          named_bar_sync(7, kSetThreads);   // last_flag may be rewritten by the next segment only after all have read it
+        }
+        if (store) {
+          if (p.y_f32) {
+            float* y = reinterpret_cast<float*>(p.y);
 #pragma unroll
             for (int m = 0; m < CW; ++m)
-              if (m < mvalid) acc[m] += __ldcg(src + m * kTileN + row);
+              if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = acc[m];
+          } else {
+            __nv_bfloat16* y = reinterpret_cast<__nv_bfloat16*>(p.y);
+#pragma unroll
+            for (int m = 0; m < CW; ++m)
+              if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = __float2bfloat16_rn(acc[m]);
           }
         }
-        named_bar_sync(3, kEpiThreads);   // last_flag may be rewritten by the next segment only after all have read it
       }
-      if (store) {
-        if (p.y_f32) {
-          float* y = reinterpret_cast<float*>(p.y);
-#pragma unroll
-          for (int m = 0; m < CW; ++m)
-            if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = acc[m];
-        } else {
-          __nv_bfloat16* y = reinterpret_cast<__nv_bfloat16*>(p.y);
-#pragma unroll
-          for (int m = 0; m < CW; ++m)
-            if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = __float2bfloat16_rn(acc[m]);
-        }
-      }
-      ER_TR(3);
       it = it_end;
+      ++seg;
     }
   }
 
-  ER_TR(5);
+  ER_TR(7);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
   if (warp == 1) tmem_dealloc<kTmemCols>(tmem);
-  ER_TR(6);
 #ifdef ER_GEMM_TRACE
   if (p.trace && blockIdx.x == p.dbg_cta && lane == 0)
     for (int i = 0; i < 8; ++i) p.trace[warp * 8 + i] = tr_sum[i];
@@ -453,6 +505,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
 }
 
 }  // namespace
+
 
 // =====================================================================================================
 // host side: tensor maps, stream-K plan, launch
