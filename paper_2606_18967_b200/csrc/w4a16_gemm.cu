@@ -73,7 +73,8 @@ struct GemmParams {
   int ntiles;          // N / 128
   int tiles;           // ntiles * mchunks
   int unit_groups;     // groups per scheduling unit: 1 (stream-K) or G (whole tiles)
-  long long units;     // tiles * G / unit_groups
+  int units;           // tiles * G / unit_groups (< 2^31, checked on the host)
+  int uq, ur;          // units / CTAs and units % CTAs: CTA c owns units [c*uq + min(c, ur), ...)
   int y_f32;
   int64_t ldy;
   void* y;
@@ -164,14 +165,13 @@ __device__ __forceinline__ void sts_f32(uint32_t saddr, float v) {
 
 __device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
-// first unit of CTA c when `units` units are dealt to `P` CTAs as contiguous, balanced ranges
-__device__ __forceinline__ long long range_begin(long long units, int P, int c) { return (units * c) / P; }
+// first unit of CTA c when the units are dealt to the CTAs as contiguous, balanced ranges (the first `ur` CTAs
+// get uq + 1 units, the others uq); 32-bit arithmetic only
+__device__ __forceinline__ int range_begin(int uq, int ur, int c) { return c * uq + min(c, ur); }
 // the CTA whose range contains unit u
-__device__ __forceinline__ int owner_of(long long units, int P, long long u) {
-  int c = (int)((u * P) / units);
-  while (c + 1 < P && range_begin(units, P, c + 1) <= u) ++c;
-  while (c > 0 && range_begin(units, P, c) > u) --c;
-  return c;
+__device__ __forceinline__ int owner_of(int uq, int ur, int u) {
+  const int big = ur * (uq + 1);
+  return u < big ? u / (uq + 1) : ur + (u - big) / uq;
 }
 
 __device__ __forceinline__ void named_bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
@@ -197,8 +197,8 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   const int lane = threadIdx.x & 31;
   const int P = gridDim.x, cta = blockIdx.x;
   const int ug = p.unit_groups;
-  const long long gb = range_begin(p.units, P, cta) * ug;        // first global group index of this CTA
-  const long long ge = range_begin(p.units, P, cta + 1) * ug;
+  const int gb = range_begin(p.uq, p.ur, cta) * ug;        // first global group index of this CTA
+  const int ge = range_begin(p.uq, p.ur, cta + 1) * ug;
   const int n_it = (int)(ge - gb);
 #ifdef ER_GEMM_TRACE
   unsigned tr_sum[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -362,9 +362,26 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
       if (kBuf == 2) rbuf ^= 1;
     };
 
+    int pend_tile[2] = {-1, -1};           // partial tiles of this CTA (head / tail segment of its range)
+    auto store_tile = [&](int tile, const float (&v)[CW]) {
+      const int n = (tile % p.ntiles) * kTileN + row, m0 = (tile / p.ntiles) * MPAD + half * CW;
+      const int mvalid = min(CW, p.M - m0);     // may be <= 0: nothing of this half is a real batch row
+      if (p.y_f32) {
+        float* y = reinterpret_cast<float*>(p.y);
+#pragma unroll
+        for (int m = 0; m < CW; ++m)
+          if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = v[m];
+      } else {
+        __nv_bfloat16* y = reinterpret_cast<__nv_bfloat16*>(p.y);
+#pragma unroll
+        for (int m = 0; m < CW; ++m)
+          if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = __float2bfloat16_rn(v[m]);
+      }
+    };
+
     while (it < n_it) {
       // ---- segment = the part of one tile inside this CTA's range ----
-      const long long gi0 = gb + it;
+      const int gi0 = gb + it;
       const int tile = (int)(gi0 / p.G), g_lo = (int)(gi0 % p.G);
       const int seg_len = min(p.G - g_lo, n_it - it);
       const int it_end = it + seg_len;
@@ -436,60 +453,81 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
         }
         if (!last_seg) named_bar_arrive(5, kThreads - kSetWarp0 * 32);
 
-        // ---- output: direct store, or partial + last-arriver reduction in ascending CTA order ----
-        const int n0 = (tile % p.ntiles) * kTileN, m0 = (tile / p.ntiles) * MPAD + half * CW;
-        const int mvalid = min(CW, p.M - m0);     // may be <= 0: nothing of this half is a real batch row
-        const int n = n0 + row;
-        bool store = true;
-        if (seg_len != p.G) {
-          float* mine = p.partials + ((size_t)cta * 2 + (it == 0 ? 0 : 1)) * (MPAD * kTileN) + half * CW * kTileN;
+        // ---- output: a whole tile is stored directly; a partial one goes to the workspace as fp32 and is
+        //      finished after the main loop (the reduction's round trips would otherwise stall the pipeline) ----
+        if (seg_len == p.G) {
+          store_tile(tile, acc);
+        } else {
+          const int k = (it == 0 ? 0 : 1);
+          const int m0 = (tile / p.ntiles) * MPAD + half * CW;
+          const int mvalid = min(CW, p.M - m0);
+          float* mine = p.partials + ((size_t)cta * 2 + k) * (MPAD * kTileN) + half * CW * kTileN;
 #pragma unroll
           for (int m = 0; m < CW; ++m)
             if (m < mvalid) __stcg(mine + m * kTileN + row, acc[m]);
-          __threadfence();
-          named_bar_sync(7, kSetThreads);
-          const long long u_first = ((long long)tile * p.G) / ug, u_last = ((long long)(tile + 1) * p.G - 1) / ug;
-          const int c_lo = owner_of(p.units, P, u_first), c_hi = owner_of(p.units, P, u_last);
-          if (leader) {
-            const int old = atomicAdd(p.counters + tile, 1);
-            const int last = (old == c_hi - c_lo);
-            if (last) p.counters[tile] = 0;  // leave the counter zero for the next call
-            *last_flag = last;
-          }
-          named_bar_sync(7, kSetThreads);
-          store = (*last_flag != 0);
-          if (store) {
-            __threadfence();
-#pragma unroll
-            for (int m = 0; m < CW; ++m) acc[m] = 0.f;
-            for (int c = c_lo; c <= c_hi; ++c) {
-              // CTA c's piece of this tile is its first segment iff its range starts inside the tile
-              const long long cb = range_begin(p.units, P, c) * ug;
-              const int which = (cb >= (long long)tile * p.G) ? 0 : 1;
-              const float* src = p.partials + ((size_t)c * 2 + which) * (MPAD * kTileN) + half * CW * kTileN;
-#pragma unroll
-              for (int m = 0; m < CW; ++m)
-                if (m < mvalid) acc[m] += __ldcg(src + m * kTileN + row);
-            }
-          }
-          named_bar_sync(7, kSetThreads);   // last_flag may be rewritten by the next segment only after all have read it
-        }
-        if (store) {
-          if (p.y_f32) {
-            float* y = reinterpret_cast<float*>(p.y);
-#pragma unroll
-            for (int m = 0; m < CW; ++m)
-              if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = acc[m];
-          } else {
-            __nv_bfloat16* y = reinterpret_cast<__nv_bfloat16*>(p.y);
-#pragma unroll
-            for (int m = 0; m < CW; ++m)
-              if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = __float2bfloat16_rn(acc[m]);
-          }
+          pend_tile[k] = tile;
         }
       }
       it = it_end;
       ++seg;
+    }
+
+    // ---- partial tiles: ticket per tile; the last CTA to arrive adds all partials in ascending CTA order ----
+    if (set == 0 && (pend_tile[0] >= 0 || pend_tile[1] >= 0)) {
+      __threadfence();
+      named_bar_sync(7, kSetThreads);
+      int c_lo[2] = {0, 0}, c_hi[2] = {-1, -1};
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        if (pend_tile[k] < 0) continue;
+        const int u_first = (pend_tile[k] * p.G) / ug;
+        const int u_last = ((pend_tile[k] + 1) * p.G - 1) / ug;
+        c_lo[k] = owner_of(p.uq, p.ur, u_first);
+        c_hi[k] = owner_of(p.uq, p.ur, u_last);
+      }
+      if (leader) {
+        int old[2] = {0, 0};
+#pragma unroll
+        for (int k = 0; k < 2; ++k)
+          if (pend_tile[k] >= 0) old[k] = atomicAdd(p.counters + pend_tile[k], 1);   // two independent round trips
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          const int last = (pend_tile[k] >= 0 && old[k] == c_hi[k] - c_lo[k]);
+          if (last) p.counters[pend_tile[k]] = 0;  // leave the counter zero for the next call
+          last_flag[k] = last;
+        }
+      }
+      named_bar_sync(7, kSetThreads);
+      constexpr int kChunk = CW <= 8 ? 4 : (CW <= 16 ? 2 : 1);   // contributors whose loads are in flight together
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        if (pend_tile[k] < 0 || last_flag[k] == 0) continue;
+        __threadfence();
+        const int tile = pend_tile[k];
+        const int m0 = (tile / p.ntiles) * MPAD + half * CW;
+        const int mvalid = min(CW, p.M - m0);
+#pragma unroll
+        for (int m = 0; m < CW; ++m) acc[m] = 0.f;
+        for (int c0 = c_lo[k]; c0 <= c_hi[k]; c0 += kChunk) {
+          float v[kChunk][CW];
+#pragma unroll
+          for (int j = 0; j < kChunk; ++j) {
+            const int c = min(c0 + j, c_hi[k]);
+            // CTA c's piece of this tile is its first segment iff its range starts inside the tile
+            const int cb = range_begin(p.uq, p.ur, c) * ug;
+            const int which = (cb >= tile * p.G) ? 0 : 1;
+            const float* src = p.partials + ((size_t)c * 2 + which) * (MPAD * kTileN) + half * CW * kTileN;
+#pragma unroll
+            for (int m = 0; m < CW; ++m) v[j][m] = (m < mvalid && c0 + j <= c_hi[k]) ? __ldcg(src + m * kTileN + row) : 0.f;
+          }
+#pragma unroll
+          for (int j = 0; j < kChunk; ++j)
+#pragma unroll
+            for (int m = 0; m < CW; ++m)
+              if (c0 + j <= c_hi[k]) acc[m] += v[j][m];
+        }
+        store_tile(tile, acc);
+      }
     }
   }
 
@@ -632,6 +670,7 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
   if (!workspace) return ER_ERR_WORKSPACE;
   if (!er::aligned16(workspace)) return ER_ERR_ALIGN;
   const Plan pl = make_plan(M, N, K);
+  if ((long long)pl.tiles * pl.G >= (1ll << 31)) return ER_ERR_SHAPE;
   if (workspace_bytes < workspace_for(pl.mpad)) return ER_ERR_WORKSPACE;
   int st = er::check_arch();
   if (st != ER_OK) return st;
@@ -645,7 +684,8 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
   }
   GemmParams gp;
   gp.M = (int)M; gp.N = (int)N; gp.K = (int)K;
-  gp.G = pl.G; gp.ntiles = pl.ntiles; gp.tiles = pl.tiles; gp.unit_groups = pl.unit_groups; gp.units = pl.units;
+  gp.G = pl.G; gp.ntiles = pl.ntiles; gp.tiles = pl.tiles; gp.unit_groups = pl.unit_groups; gp.units = (int)pl.units;
+  gp.uq = (int)(pl.units / pl.ctas); gp.ur = (int)(pl.units % pl.ctas);
   gp.dbg = g_tune_dbg;
 #ifdef ER_GEMM_TRACE
   gp.trace = g_trace;
