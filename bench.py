@@ -38,8 +38,8 @@ REFRESH_BYTES_PER_ELEM = 2.0 + W4_BYTES_PER_WEIGHT
 LAYER_COPIES = 4
 VERIFY_B, VERIFY_GAMMA, VERIFY_V = 64, 4, 152064
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (w4a16_gemm_kernel<16>,
-# gate_up at M=16) from the ncu --set full capture summarised in profiles/; None until captured.
-NCU_TRAFFIC_BYTES = None
+# all M<=16 launches of one step) from the ncu --set full capture summarised in profiles/r01_v4_ncu.md.
+NCU_TRAFFIC_BYTES = 30.3e6   # mean over the 20 M<=16 launches of profiles/r01_v4_ncu.md (algorithmic: 30.29e6)
 
 
 def log(*a):
