@@ -3,60 +3,91 @@
 // adjusted target distribution", bonus token when everything is accepted; L544: needs the full
 // distribution at the rejected position).
 //
-// One CTA of 1024 threads per sequence.  Rows of the vocabulary are streamed with 128-bit loads in tiles
-// of 8192 elements (8 consecutive elements per thread).  The accept scan is lazy: position i's softmax
-// normalisers are only computed if positions < i were all accepted, so a sequence rejected at position n
-// reads 2 (n + 1) rows instead of 2 gamma + 1.  The residual draw is a two-level inverse CDF: per-warp
-// segment sums (256 consecutive tokens) -> fp64 prefix over segments by one thread -> warp scan inside
-// the one segment that contains the threshold.
+// One thread-block CLUSTER (up to 8 CTAs of 256 threads) per sequence: with one CTA per sequence only B of
+// the 148 SMs pull bytes (9 % DRAM throughput measured at B = 64, profiles/r01_baseline_ncu.md).  Every CTA
+// owns a contiguous range of 2048-token tiles of the vocabulary; rows are streamed with 128-bit loads (8
+// consecutive elements per thread).  Per-row softmax normalisers and residual masses are reduced inside the
+// CTA, exchanged through distributed shared memory and combined in rank order by every CTA, so all CTAs of
+// a cluster take the same decisions.  The accept scan is lazy: position i's normalisers are only computed if
+// positions < i were all accepted, so a sequence rejected at position n reads 2 (n + 1) rows instead of
+// 2 gamma + 1.  The residual draw is a multi-level inverse CDF: per-warp segment sums (256 consecutive
+// tokens) -> per-CTA totals, exchanged -> the CTA whose range holds the threshold does an fp64 prefix over
+// its segments and a warp scan inside the one segment that contains the threshold.
+#include <cooperative_groups.h>
 #include "er_common.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace {
 
-constexpr int kThreads = 1024;
+constexpr int kThreads = 256;
+constexpr int kMaxCluster = 8;
 constexpr int kWarps = kThreads / 32;
 constexpr int kPerThread = 8;
-constexpr int kTile = kThreads * kPerThread;  // 8192 tokens
+constexpr int kTile = kThreads * kPerThread;  // 2048 tokens
 constexpr int kMaxV = 1 << 20;
 constexpr float kNegInf = -3.0e38f;
 
-// ---- 8 consecutive elements starting at token v0 (clipped to V), widened to fp32 -------------
+// ---- 8 consecutive elements starting at token v0 (clipped to V): raw load, then widening to fp32 ----
+// (split in two so that the loads of several tiles can be in flight before the first one is consumed)
 template <typename T>
 struct Load8;
 template <>
 struct Load8<float> {
-  static __device__ __forceinline__ void run(const float* row, int v0, int V, bool vec, float fill, float (&f)[8]) {
+  struct Raw { float4 a, b; };
+  static constexpr int kBatch = 2;   // tiles whose loads are issued together
+  static __device__ __forceinline__ Raw load(const float* row, int v0, int V, bool vec, float fill) {
+    Raw r;
     if (vec && v0 + 8 <= V) {
-      const float4 a = *reinterpret_cast<const float4*>(row + v0);
-      const float4 b = *reinterpret_cast<const float4*>(row + v0 + 4);
-      f[0] = a.x; f[1] = a.y; f[2] = a.z; f[3] = a.w;
-      f[4] = b.x; f[5] = b.y; f[6] = b.z; f[7] = b.w;
+      r.a = *reinterpret_cast<const float4*>(row + v0);
+      r.b = *reinterpret_cast<const float4*>(row + v0 + 4);
     } else {
+      float f[8];
 #pragma unroll
       for (int i = 0; i < 8; ++i) f[i] = (v0 + i < V) ? row[v0 + i] : fill;
+      r.a = make_float4(f[0], f[1], f[2], f[3]);
+      r.b = make_float4(f[4], f[5], f[6], f[7]);
     }
+    return r;
+  }
+  static __device__ __forceinline__ void expand(const Raw& r, float (&f)[8]) {
+    f[0] = r.a.x; f[1] = r.a.y; f[2] = r.a.z; f[3] = r.a.w;
+    f[4] = r.b.x; f[5] = r.b.y; f[6] = r.b.z; f[7] = r.b.w;
   }
   static __device__ __forceinline__ float one(const float* row, int v) { return row[v]; }
 };
 template <>
 struct Load8<__nv_bfloat16> {
-  static __device__ __forceinline__ void run(const __nv_bfloat16* row, int v0, int V, bool vec, float fill,
-                                             float (&f)[8]) {
+  struct Raw { uint4 a; };
+  static constexpr int kBatch = 4;
+  static __device__ __forceinline__ Raw load(const __nv_bfloat16* row, int v0, int V, bool vec, float fill) {
+    Raw r;
     if (vec && v0 + 8 <= V) {
-      const uint4 a = *reinterpret_cast<const uint4*>(row + v0);
-      const uint32_t r[4] = {a.x, a.y, a.z, a.w};
-#pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        f[2 * i] = __uint_as_float(r[i] << 16);
-        f[2 * i + 1] = __uint_as_float(r[i] & 0xFFFF0000u);
-      }
+      r.a = *reinterpret_cast<const uint4*>(row + v0);
     } else {
+      uint32_t h[8];
+      const uint32_t fb = __float_as_uint(fill) >> 16;   // the fills used (0, -3e38) survive truncation to bf16
 #pragma unroll
-      for (int i = 0; i < 8; ++i) f[i] = (v0 + i < V) ? __bfloat162float(row[v0 + i]) : fill;
+      for (int i = 0; i < 8; ++i)
+        h[i] = (v0 + i < V) ? (uint32_t)__bfloat16_as_ushort(row[v0 + i]) : fb;
+      r.a = make_uint4(h[0] | (h[1] << 16), h[2] | (h[3] << 16), h[4] | (h[5] << 16), h[6] | (h[7] << 16));
+    }
+    return r;
+  }
+  static __device__ __forceinline__ void expand(const Raw& r, float (&f)[8]) {
+    const uint32_t w[4] = {r.a.x, r.a.y, r.a.z, r.a.w};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      f[2 * i] = __uint_as_float(w[i] << 16);
+      f[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
     }
   }
   static __device__ __forceinline__ float one(const __nv_bfloat16* row, int v) { return __bfloat162float(row[v]); }
 };
+template <typename T>
+__device__ __forceinline__ void load8(const T* row, int v0, int V, bool vec, float fill, float (&f)[8]) {
+  Load8<T>::expand(Load8<T>::load(row, v0, V, vec, fill), f);
+}
 
 __device__ __forceinline__ float warp_max(float x) {
 #pragma unroll
@@ -75,8 +106,11 @@ struct RowStats {
 };
 
 struct Shared {
+  float4 xstats[2][kMaxCluster];   // [parity][rank]: (max_t, sum_t, max_d, sum_d) of every CTA's vocabulary range
+  double xmass[2][kMaxCluster];    // [parity][rank]: residual mass of every CTA's range
   float red_a[kWarps];
   float red_b[kWarps];
+  float px[16], qx[16], ua[16];    // target / draft value at the drafted token and the uniform, per position
   float bc[4];
   int seg;
   int token;
@@ -84,65 +118,107 @@ struct Shared {
   double thr_local;
 };
 
-// Softmax normalisers of one target row and (optionally) one draft row in a single pass; online max/sum.
+struct ClusterCtx {
+  int rank, size;      // this CTA's rank in the cluster, CTAs per cluster
+  int tile_lo, tile_hi;  // its range of kTile-token tiles
+  int xpar;            // parity of the next exchange buffer
+};
+
+// Softmax normalisers of one target row and (optionally) one draft row in a single pass over this CTA's tile
+// range (online max/sum), then combined over the cluster in rank order: identical in every CTA.
 template <typename T>
-__device__ void row_stats(const T* trow, const T* drow, int V, bool vec, float scale, Shared& sh, RowStats& st,
-                          RowStats& sd) {
+__device__ void row_stats(const T* trow, const T* drow, int V, bool vec, float scale, Shared& sh, ClusterCtx& cx,
+                          RowStats& st, RowStats& sd) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   float mt = kNegInf, st_ = 0.f, md = kNegInf, sd_ = 0.f;
-  for (int base = 0; base < V; base += kTile) {
-    const int v0 = base + tid * kPerThread;
-    if (v0 >= V) break;
-    float f[8];
-    Load8<T>::run(trow, v0, V, vec, kNegInf, f);
-    float cm = f[0];
+  constexpr int NB = Load8<T>::kBatch;
+  for (int t0 = cx.tile_lo; t0 < cx.tile_hi; t0 += NB) {
+    typename Load8<T>::Raw rt[NB], rd[NB];
 #pragma unroll
-    for (int i = 1; i < 8; ++i) cm = fmaxf(cm, f[i]);
-    if (cm > mt) { st_ *= exp2f((mt - cm) * scale); mt = cm; }
+    for (int j = 0; j < NB; ++j) {           // all loads of the batch first: they overlap in flight
+      const int v0 = (t0 + j) * kTile + tid * kPerThread;
+      if (t0 + j < cx.tile_hi && v0 < V) {
+        rt[j] = Load8<T>::load(trow, v0, V, vec, kNegInf);
+        if (drow) rd[j] = Load8<T>::load(drow, v0, V, vec, kNegInf);
+      }
+    }
 #pragma unroll
-    for (int i = 0; i < 8; ++i) st_ += exp2f((f[i] - mt) * scale);
-    if (drow) {
-      Load8<T>::run(drow, v0, V, vec, kNegInf, f);
-      cm = f[0];
+    for (int j = 0; j < NB; ++j) {
+      const int v0 = (t0 + j) * kTile + tid * kPerThread;
+      if (t0 + j < cx.tile_hi && v0 < V) {
+        float f[8];
+        Load8<T>::expand(rt[j], f);
+        float cm = f[0];
 #pragma unroll
-      for (int i = 1; i < 8; ++i) cm = fmaxf(cm, f[i]);
-      if (cm > md) { sd_ *= exp2f((md - cm) * scale); md = cm; }
+        for (int i = 1; i < 8; ++i) cm = fmaxf(cm, f[i]);
+        if (cm > mt) { st_ *= exp2f((mt - cm) * scale); mt = cm; }
 #pragma unroll
-      for (int i = 0; i < 8; ++i) sd_ += exp2f((f[i] - md) * scale);
+        for (int i = 0; i < 8; ++i) st_ += exp2f((f[i] - mt) * scale);
+        if (drow) {
+          Load8<T>::expand(rd[j], f);
+          cm = f[0];
+#pragma unroll
+          for (int i = 1; i < 8; ++i) cm = fmaxf(cm, f[i]);
+          if (cm > md) { sd_ *= exp2f((md - cm) * scale); md = cm; }
+#pragma unroll
+          for (int i = 0; i < 8; ++i) sd_ += exp2f((f[i] - md) * scale);
+        }
+      }
     }
   }
-  // block max
+  // CTA max
   float wm_t = warp_max(mt), wm_d = warp_max(md);
   if (lane == 0) { sh.red_a[warp] = wm_t; sh.red_b[warp] = wm_d; }
   __syncthreads();
-  float bm_t = sh.red_a[lane], bm_d = sh.red_b[lane];
+  float bm_t = lane < kWarps ? sh.red_a[lane] : kNegInf, bm_d = lane < kWarps ? sh.red_b[lane] : kNegInf;
   bm_t = warp_max(bm_t); bm_d = warp_max(bm_d);
   __syncthreads();
-  // block sum of rescaled partial sums
+  // CTA sum of rescaled partial sums
   st_ = (mt > kNegInf) ? st_ * exp2f((mt - bm_t) * scale) : 0.f;
   sd_ = (md > kNegInf) ? sd_ * exp2f((md - bm_d) * scale) : 0.f;
   float ws_t = warp_sum(st_), ws_d = warp_sum(sd_);
   if (lane == 0) { sh.red_a[warp] = ws_t; sh.red_b[warp] = ws_d; }
   __syncthreads();
-  float bs_t = warp_sum(sh.red_a[lane]), bs_d = warp_sum(sh.red_b[lane]);
-  __syncthreads();
-  st.max = bm_t; st.inv_sum = __fdiv_rn(1.0f, bs_t);
-  sd.max = bm_d; sd.inv_sum = drow ? __fdiv_rn(1.0f, bs_d) : 0.f;
+  float bs_t = warp_sum(lane < kWarps ? sh.red_a[lane] : 0.f), bs_d = warp_sum(lane < kWarps ? sh.red_b[lane] : 0.f);
+  // cluster: every CTA publishes its (max, sum) pair to all CTAs, then all combine in rank order
+  cg::cluster_group cluster = cg::this_cluster();
+  const int par = cx.xpar;
+  cx.xpar ^= 1;
+  if (tid < cx.size) {
+    float4* dst = cluster.map_shared_rank(&sh.xstats[par][cx.rank], tid);
+    *dst = make_float4(bm_t, bs_t, bm_d, bs_d);
+  }
+  cluster.sync();
+  float gm_t = kNegInf, gm_d = kNegInf;
+  for (int c = 0; c < cx.size; ++c) {
+    gm_t = fmaxf(gm_t, sh.xstats[par][c].x);
+    gm_d = fmaxf(gm_d, sh.xstats[par][c].z);
+  }
+  float gs_t = 0.f, gs_d = 0.f;
+  for (int c = 0; c < cx.size; ++c) {
+    const float4 v = sh.xstats[par][c];
+    if (v.x > kNegInf) gs_t += v.y * exp2f((v.x - gm_t) * scale);
+    if (v.z > kNegInf) gs_d += v.w * exp2f((v.z - gm_d) * scale);
+  }
+  st.max = gm_t; st.inv_sum = __fdiv_rn(1.0f, gs_t);
+  sd.max = gm_d; sd.inv_sum = drow ? __fdiv_rn(1.0f, gs_d) : 0.f;
 }
 
-// The 8 residual weights of one thread chunk.  use_q == false: w = p (bonus token / degenerate residual).
+// The 8 residual weights of one thread chunk from its raw loads.  use_q == false: w = p (bonus token /
+// degenerate residual).
 template <typename T, bool kLogits>
-__device__ __forceinline__ void weights8(const T* trow, const T* drow, int v0, int V, bool vec, float scale,
-                                         const RowStats& st, const RowStats& sd, bool use_q, float (&w)[8]) {
+__device__ __forceinline__ void weights8_raw(const typename Load8<T>::Raw& rp, const typename Load8<T>::Raw& rq,
+                                             float scale, const RowStats& st, const RowStats& sd, bool use_q,
+                                             float (&w)[8]) {
   float p[8];
-  Load8<T>::run(trow, v0, V, vec, kLogits ? kNegInf : 0.f, p);
+  Load8<T>::expand(rp, p);
   if (kLogits) {
 #pragma unroll
     for (int i = 0; i < 8; ++i) p[i] = exp2f((p[i] - st.max) * scale) * st.inv_sum;
   }
   if (use_q) {
     float q[8];
-    Load8<T>::run(drow, v0, V, vec, kLogits ? kNegInf : 0.f, q);
+    Load8<T>::expand(rq, q);
     if (kLogits) {
 #pragma unroll
       for (int i = 0; i < 8; ++i) q[i] = exp2f((q[i] - sd.max) * scale) * sd.inv_sum;
@@ -154,57 +230,103 @@ __device__ __forceinline__ void weights8(const T* trow, const T* drow, int v0, i
     for (int i = 0; i < 8; ++i) w[i] = p[i];
   }
 }
+template <typename T, bool kLogits>
+__device__ __forceinline__ void weights8(const T* trow, const T* drow, int v0, int V, bool vec, float scale,
+                                         const RowStats& st, const RowStats& sd, bool use_q, float (&w)[8]) {
+  const float fill = kLogits ? kNegInf : 0.f;
+  typename Load8<T>::Raw rp = Load8<T>::load(trow, v0, V, vec, fill), rq = rp;
+  if (use_q) rq = Load8<T>::load(drow, v0, V, vec, fill);
+  weights8_raw<T, kLogits>(rp, rq, scale, st, sd, use_q, w);
+}
 
-// Inverse-CDF draw over w in vocab order: token = min{v : C(v) > r R}.  Returns -1 if R == 0.
+// Inverse-CDF draw over w in vocab order: token = min{v : C(v) > r R}.  Returns -1 in every CTA of the cluster
+// if R == 0; otherwise the token in the CTA whose tile range holds the threshold and -2 in the others.
 template <typename T, bool kLogits>
 __device__ int draw_token(const T* trow, const T* drow, int V, bool vec, float scale, const RowStats& st,
-                          const RowStats& sd, bool use_q, float r, Shared& sh, float* seg_sums) {
+                          const RowStats& sd, bool use_q, float r, Shared& sh, ClusterCtx& cx, float* seg_sums) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int tiles = (V + kTile - 1) / kTile;
-  // level 1: sums of 256-token segments (one warp, one tile each)
-  for (int t = 0; t < tiles; ++t) {
-    const int v0 = t * kTile + tid * kPerThread;
-    float s = 0.f;
-    if (v0 < V) {
-      float w[8];
-      weights8<T, kLogits>(trow, drow, v0, V, vec, scale, st, sd, use_q, w);
-      s = ((w[0] + w[1]) + (w[2] + w[3])) + ((w[4] + w[5]) + (w[6] + w[7]));
+  const int ntile = cx.tile_hi - cx.tile_lo;
+  // level 1: sums of 256-token segments (one warp, one tile each) of this CTA's range
+  constexpr int NB = Load8<T>::kBatch;
+  const float fill = kLogits ? kNegInf : 0.f;
+  for (int t0 = 0; t0 < ntile; t0 += NB) {
+    typename Load8<T>::Raw rp[NB], rq[NB];
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {           // all loads of the batch first: they overlap in flight
+      const int v0 = (cx.tile_lo + t0 + j) * kTile + tid * kPerThread;
+      if (t0 + j < ntile && v0 < V) {
+        rp[j] = Load8<T>::load(trow, v0, V, vec, fill);
+        if (use_q) rq[j] = Load8<T>::load(drow, v0, V, vec, fill);
+      }
     }
-    s = warp_sum(s);
-    if (lane == 0) seg_sums[t * kWarps + warp] = s;
+#pragma unroll
+    for (int j = 0; j < NB; ++j) {
+      if (t0 + j < ntile) {                  // uniform over the CTA
+        const int v0 = (cx.tile_lo + t0 + j) * kTile + tid * kPerThread;
+        float s = 0.f;
+        if (v0 < V) {
+          float w[8];
+          weights8_raw<T, kLogits>(rp[j], use_q ? rq[j] : rp[j], scale, st, sd, use_q, w);
+          s = ((w[0] + w[1]) + (w[2] + w[3])) + ((w[4] + w[5]) + (w[6] + w[7]));
+        }
+        s = warp_sum(s);
+        if (lane == 0) seg_sums[(t0 + j) * kWarps + warp] = s;
+      }
+    }
   }
   __syncthreads();
-  // level 2: fp64 prefix over segments in vocab order by one thread
-  if (tid == 0) {
-    const int nseg = tiles * kWarps;
-    double R = 0.0;
-    for (int i = 0; i < nseg; ++i) R += (double)seg_sums[i];
-    int seg = -1;
-    double excl = 0.0;
-    if (R > 0.0) {
-      const double thr = (double)r * R;
-      double c = 0.0;
-      seg = nseg - 1;
-      for (int i = 0; i < nseg; ++i) {
-        const double nc = c + (double)seg_sums[i];
-        if (nc > thr) { seg = i; break; }
-        c = nc;
-      }
-      // if rounding left no segment (cannot happen for r < 1), fall to the last segment with mass
-      while (seg > 0 && !(seg_sums[seg] > 0.f)) --seg;
-      excl = 0.0;
-      for (int i = 0; i < seg; ++i) excl += (double)seg_sums[i];
-      sh.thr_local = thr - excl;
+  // level 2a: this CTA's mass (fp64, vocab order), published to the whole cluster
+  cg::cluster_group cluster = cg::this_cluster();
+  const int par = cx.xpar;
+  cx.xpar ^= 1;
+  const int nseg = ntile * kWarps;
+  if (warp == 0) {
+    double mine = 0.0;
+    for (int i = 0; i < nseg; ++i) mine += (double)seg_sums[i];   // every lane: the same sequential sum
+    if (lane < cx.size) *cluster.map_shared_rank(&sh.xmass[par][cx.rank], lane) = mine;
+  }
+  cluster.sync();
+  // level 2b: every CTA finds, identically, the rank whose range holds the threshold
+  double R = 0.0;
+  for (int c = 0; c < cx.size; ++c) R += sh.xmass[par][c];
+  if (!(R > 0.0)) return -1;
+  const double thr = (double)r * R;
+  int owner = cx.size - 1;
+  double before = 0.0;
+  {
+    double c0 = 0.0;
+    for (int c = 0; c < cx.size; ++c) {
+      const double nc = c0 + sh.xmass[par][c];
+      if (nc > thr) { owner = c; break; }
+      c0 = nc;
     }
+    // if rounding left no rank (cannot happen for r < 1), fall to the last rank with mass
+    while (owner > 0 && !(sh.xmass[par][owner] > 0.0)) --owner;
+    for (int c = 0; c < owner; ++c) before += sh.xmass[par][c];
+  }
+  if (owner != cx.rank) return -2;
+  // level 2c (owner only): fp64 prefix over its segments in vocab order by one thread
+  if (tid == 0) {
+    const double thr_cta = thr - before;
+    double c = 0.0;
+    int seg = nseg - 1;
+    for (int i = 0; i < nseg; ++i) {
+      const double nc = c + (double)seg_sums[i];
+      if (nc > thr_cta) { seg = i; break; }
+      c = nc;
+    }
+    while (seg > 0 && !(seg_sums[seg] > 0.f)) --seg;
+    double excl = 0.0;
+    for (int i = 0; i < seg; ++i) excl += (double)seg_sums[i];
+    sh.thr_local = thr_cta - excl;
     sh.seg = seg;
     sh.token = -1;
   }
   __syncthreads();
   const int seg = sh.seg;
-  if (seg < 0) return -1;
   // level 3: warp scan inside the chosen 256-token segment
   if (warp == 0) {
-    const int v0 = (seg / kWarps) * kTile + (seg % kWarps) * 256 + lane * kPerThread;
+    const int v0 = (cx.tile_lo + seg / kWarps) * kTile + (seg % kWarps) * 256 + lane * kPerThread;
     float w[8];
 #pragma unroll
     for (int i = 0; i < 8; ++i) w[i] = 0.f;
@@ -246,34 +368,49 @@ __device__ int draw_token(const T* trow, const T* drow, int V, bool vec, float s
 }
 
 template <typename T, bool kLogits>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kThreads, 4)
 spec_verify_kernel(const T* __restrict__ target, const T* __restrict__ draft, float scale,
                    const int32_t* __restrict__ draft_tokens, const float* __restrict__ u_accept,
                    const float* __restrict__ u_sample, int gamma, int V, int32_t* __restrict__ accept_count,
                    int32_t* __restrict__ out_tokens) {
   extern __shared__ float seg_sums[];
   __shared__ Shared sh;
-  const int b = blockIdx.x, tid = threadIdx.x;
+  cg::cluster_group cluster = cg::this_cluster();
+  ClusterCtx cx;
+  cx.size = (int)cluster.num_blocks();
+  cx.rank = (int)cluster.block_rank();
+  cx.xpar = 0;
+  const int tiles = (V + kTile - 1) / kTile;
+  const int per = (tiles + cx.size - 1) / cx.size;
+  cx.tile_lo = min(cx.rank * per, tiles);
+  cx.tile_hi = min(cx.tile_lo + per, tiles);
+  const int b = blockIdx.x / cx.size, tid = threadIdx.x;
   const bool vec = ((size_t)V * sizeof(T)) % 16 == 0;
   const T* tgt = target + (size_t)b * (gamma + 1) * V;
   const T* drf = draft + (size_t)b * gamma * V;
   const int32_t* xs = draft_tokens + (size_t)b * gamma;
+
+  if (tid < gamma) {           // everything the accept tests read, fetched once, off the per-position critical path
+    const int x = min(max(xs[tid], 0), V - 1);
+    sh.px[tid] = Load8<T>::one(tgt + (size_t)tid * V, x);
+    sh.qx[tid] = Load8<T>::one(drf + (size_t)tid * V, x);
+    sh.ua[tid] = u_accept[(size_t)b * gamma + tid];
+  }
+  __syncthreads();
 
   RowStats st{0.f, 1.f}, sd{0.f, 1.f};
   int n = 0;
   for (; n < gamma; ++n) {
     const T* trow = tgt + (size_t)n * V;
     const T* drow = drf + (size_t)n * V;
-    if (kLogits) row_stats<T>(trow, drow, V, vec, scale, sh, st, sd);
-    if (tid == 0) {
-      int x = xs[n];
-      x = min(max(x, 0), V - 1);
-      float p = Load8<T>::one(trow, x), q = Load8<T>::one(drow, x);
+    if (kLogits) row_stats<T>(trow, drow, V, vec, scale, sh, cx, st, sd);
+    if (tid == 0) {            // every CTA of the cluster takes the same decision from the same numbers
+      float p = sh.px[n], q = sh.qx[n];
       if (kLogits) {
         p = exp2f((p - st.max) * scale) * st.inv_sum;
         q = exp2f((q - sd.max) * scale) * sd.inv_sum;
       }
-      const float lhs = __fmul_rn(u_accept[(size_t)b * gamma + n], q);
+      const float lhs = __fmul_rn(sh.ua[n], q);
       sh.flag = (lhs < p) ? 1 : 0;
     }
     __syncthreads();
@@ -283,11 +420,12 @@ spec_verify_kernel(const T* __restrict__ target, const T* __restrict__ draft, fl
   }
   const T* trow = tgt + (size_t)n * V;
   const T* drow = (n < gamma) ? drf + (size_t)n * V : nullptr;
-  if (n == gamma && kLogits) row_stats<T>(trow, nullptr, V, vec, scale, sh, st, sd);
+  if (n == gamma && kLogits) row_stats<T>(trow, nullptr, V, vec, scale, sh, cx, st, sd);
   const float r = u_sample[b];
-  int tok = draw_token<T, kLogits>(trow, drow, V, vec, scale, st, sd, n < gamma, r, sh, seg_sums);
-  if (tok < 0) tok = draw_token<T, kLogits>(trow, nullptr, V, vec, scale, st, sd, false, r, sh, seg_sums);
-  if (tok < 0) tok = V - 1;  // all-zero target row: outside the contract, stay memory-safe
+  int tok = draw_token<T, kLogits>(trow, drow, V, vec, scale, st, sd, n < gamma, r, sh, cx, seg_sums);
+  if (tok == -1) tok = draw_token<T, kLogits>(trow, nullptr, V, vec, scale, st, sd, false, r, sh, cx, seg_sums);
+  if (tok == -1) tok = (cx.rank == 0) ? V - 1 : -2;  // all-zero target row: outside the contract, stay memory-safe
+  if (tok == -2) return;                             // another CTA of the cluster owns the draw and the outputs
   if (tid == 0) accept_count[b] = n;
   if (tid <= gamma) {
     int32_t o = -1;
@@ -295,6 +433,27 @@ spec_verify_kernel(const T* __restrict__ target, const T* __restrict__ draft, fl
     else if (tid == n) o = tok;
     out_tokens[(size_t)b * (gamma + 1) + tid] = o;
   }
+}
+
+template <typename T, bool kLogits>
+int launch_verify(int cluster_size, size_t smem, cudaStream_t s, const T* target, const T* draft, float scale,
+                  const int32_t* draft_tokens, const float* u_accept, const float* u_sample, int B, int gamma, int V,
+                  int32_t* accept_count, int32_t* out_tokens) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(B * cluster_size));
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)cluster_size;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  ER_CUDA_TRY(cudaLaunchKernelEx(&cfg, spec_verify_kernel<T, kLogits>, target, draft, scale, draft_tokens, u_accept,
+                                 u_sample, gamma, V, accept_count, out_tokens));
+  return ER_OK;
 }
 
 }  // namespace
@@ -313,22 +472,24 @@ extern "C" int er_spec_verify(const void* target, const void* draft, int in_dtyp
   int st = er::check_arch();
   if (st != ER_OK) return st;
   const int tiles = (V + kTile - 1) / kTile;
-  const size_t smem = (size_t)tiles * kWarps * sizeof(float);
+  const int cluster = tiles >= 8 ? 8 : (tiles >= 4 ? 4 : (tiles >= 2 ? 2 : 1));   // CTAs per sequence
+  const int per = (tiles + cluster - 1) / cluster;
+  const size_t smem = (size_t)per * kWarps * sizeof(float);
   const float scale = (float)(1.4426950408889634 / (double)temperature);
   cudaStream_t s = (cudaStream_t)stream;
+  int rc;
   if (in_dtype == ER_F32 && !inputs_are_logits) {
-    spec_verify_kernel<float, false><<<B, kThreads, smem, s>>>((const float*)target, (const float*)draft, scale,
-                                                               draft_tokens, u_accept, u_sample, gamma, V,
-                                                               accept_count, out_tokens);
+    rc = launch_verify<float, false>(cluster, smem, s, (const float*)target, (const float*)draft, scale, draft_tokens,
+                                     u_accept, u_sample, B, gamma, V, accept_count, out_tokens);
   } else if (in_dtype == ER_F32) {
-    spec_verify_kernel<float, true><<<B, kThreads, smem, s>>>((const float*)target, (const float*)draft, scale,
-                                                              draft_tokens, u_accept, u_sample, gamma, V,
-                                                              accept_count, out_tokens);
+    rc = launch_verify<float, true>(cluster, smem, s, (const float*)target, (const float*)draft, scale, draft_tokens,
+                                    u_accept, u_sample, B, gamma, V, accept_count, out_tokens);
   } else {
-    spec_verify_kernel<__nv_bfloat16, true><<<B, kThreads, smem, s>>>(
-        (const __nv_bfloat16*)target, (const __nv_bfloat16*)draft, scale, draft_tokens, u_accept, u_sample, gamma, V,
-        accept_count, out_tokens);
+    rc = launch_verify<__nv_bfloat16, true>(cluster, smem, s, (const __nv_bfloat16*)target,
+                                            (const __nv_bfloat16*)draft, scale, draft_tokens, u_accept, u_sample, B,
+                                            gamma, V, accept_count, out_tokens);
   }
+  if (rc != ER_OK) return rc;
   ER_CUDA_TRY(cudaGetLastError());
   return ER_OK;
 }
