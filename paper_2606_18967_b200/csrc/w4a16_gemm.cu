@@ -473,8 +473,10 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
     }
 
     // ---- partial tiles: ticket per tile; the last CTA to arrive adds all partials in ascending CTA order ----
+    // Ordering: partial stores (all threads) -> bar.sync -> the leader's acq_rel ticket (release is cumulative over
+    // what the barrier made visible to the leader); last arriver: acq_rel ticket -> bar.sync -> ld.cg of the others'
+    // partials.  No per-thread __threadfence on either side.
     if (set == 0 && (pend_tile[0] >= 0 || pend_tile[1] >= 0)) {
-      __threadfence();
       named_bar_sync(7, kSetThreads);
       int c_lo[2] = {0, 0}, c_hi[2] = {-1, -1};
 #pragma unroll
@@ -489,7 +491,8 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
         int old[2] = {0, 0};
 #pragma unroll
         for (int k = 0; k < 2; ++k)
-          if (pend_tile[k] >= 0) old[k] = atomicAdd(p.counters + pend_tile[k], 1);   // two independent round trips
+          if (pend_tile[k] >= 0)   // two independent round trips
+            asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old[k]) : "l"(p.counters + pend_tile[k]) : "memory");
 #pragma unroll
         for (int k = 0; k < 2; ++k) {
           const int last = (pend_tile[k] >= 0 && old[k] == c_hi[k] - c_lo[k]);
@@ -502,7 +505,6 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
 #pragma unroll
       for (int k = 0; k < 2; ++k) {
         if (pend_tile[k] < 0 || last_flag[k] == 0) continue;
-        __threadfence();
         const int tile = pend_tile[k];
         const int m0 = (tile / p.ntiles) * MPAD + half * CW;
         const int mvalid = min(CW, p.M - m0);

@@ -139,17 +139,14 @@ def test_split_k_counts_agree_and_are_deterministic(splits):
     assert torch.equal(y1, y2)
 
 
-@pytest.mark.parametrize("name,N,K", [("qkv", 4608, 3584), ("o", 3584, 3584), ("gate_up", 37888, 3584),
-                                      ("down", 3584, 18944)])
-@pytest.mark.parametrize("M", [1, 16, 256])
-def test_config1_full_size_sampled_columns(name, N, K, M):
-    # full 7B-layer shapes in the launch configuration bench.py times; oracle on the 256 output columns of two sampled 128-row tiles
-    w = I.weight_bf16(N, K, I.seed_of("cfg1", name), device=DEV)
-    x = I.activation_bf16(M, K, I.seed_of("cfg1", name, "x", M), device=DEV)
-    qw, sc = er.quantize_pack(w)
-    y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
+def _sampled_columns_check(x, qw, sc, N, K, seed, label, y=None):
+    """Launches the GEMM (fp32 out) and checks the 256 output columns of two sampled 128-row tiles against the
+    fp64 oracle evaluated on the same device inputs."""
+    M = x.shape[0]
+    if y is None:
+        y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
     torch.cuda.synchronize()
-    rng = np.random.default_rng(N + M)
+    rng = np.random.default_rng(seed)
     G = K // 128
     blocks = qw.view(N // 128, G * 2048)                    # ER_PACK_V2: one row of this view per 128-row tile
     tiles = np.sort(rng.choice(N // 128, size=2, replace=False))
@@ -159,5 +156,64 @@ def test_config1_full_size_sampled_columns(name, N, K, M):
     y_ref = O.w4a16_gemm(I.as_u16(x), qsel, I.as_u16(sc[:, ct].contiguous()))
     got = y[:, ct].cpu().numpy().astype(np.float64)
     err = np.abs(got - y_ref).max()
-    assert err <= _tol(y_ref), f"{name} M={M}: max|d|={err} tol={_tol(y_ref)}"
+    assert err <= _tol(y_ref), f"{label} M={M}: max|d|={err} tol={_tol(y_ref)}"
     assert torch.isfinite(y).all()
+    return y
+
+
+@pytest.mark.parametrize("name,N,K", [("qkv", 4608, 3584), ("o", 3584, 3584), ("gate_up", 37888, 3584),
+                                      ("down", 3584, 18944)])
+@pytest.mark.parametrize("M", [1, 16, 256])
+def test_config1_full_size_sampled_columns(name, N, K, M):
+    # full 7B-layer shapes in the launch configuration bench.py times
+    w = I.weight_bf16(N, K, I.seed_of("cfg1", name), device=DEV)
+    x = I.activation_bf16(M, K, I.seed_of("cfg1", name, "x", M), device=DEV)
+    qw, sc = er.quantize_pack(w)
+    _sampled_columns_check(x, qw, sc, N, K, N + M, name)
+
+
+@pytest.mark.parametrize("name,N,K", [("qkv", 7168, 5120), ("o", 5120, 5120), ("gate_up", 55296, 5120),
+                                      ("down", 5120, 27648)])
+@pytest.mark.parametrize("M", [1, 8, 32])
+def test_config4_32b_shapes_sampled_columns(name, N, K, M):
+    # BASELINE.json configs[4]: the 32B-class linears at batch 1-32
+    w = I.weight_bf16(N, K, I.seed_of("cfg4", name), device=DEV)
+    x = I.activation_bf16(M, K, I.seed_of("cfg4", name, "x", M), device=DEV)
+    qw, sc = er.quantize_pack(w)
+    del w
+    _sampled_columns_check(x, qw, sc, N, K, N + M, name)
+
+
+def test_config2_layer_chain_teacher_forced_shrinking_batch():
+    # BASELINE.json configs[2]: the linears of one 7B drafter layer chained through real data dependencies while the
+    # active batch shrinks 256 -> 1; every GEMM is checked on the input the GPU actually fed it (errors do not
+    # compound).  Glue: attention := first 3584 columns of QKV, SiLU(gate) * up, RMS renormalisation.
+    H, FF = 3584, 18944
+    shapes = {"qkv": (4608, H), "o": (H, H), "gate_up": (2 * FF, H), "down": (H, FF)}
+    W = {}
+    for n, (N, K) in shapes.items():
+        w = I.weight_bf16(N, K, I.seed_of("cfg2", n), device=DEV)
+        W[n] = er.quantize_pack(w)
+        del w
+    ws = er.gemm_workspace(256, 2 * FF, H, DEV)
+
+    def renorm(t):
+        t = t.float()
+        return (t / t.pow(2).mean(dim=1, keepdim=True).sqrt().clamp_min(1e-6)).to(torch.bfloat16)
+
+    for M in (256, 128, 64, 16, 4, 1):
+        h = I.activation_bf16(M, H, I.seed_of("cfg2", "x", M), device=DEV)
+
+        def lin(n, x):
+            N, K = shapes[n]
+            y = er.w4a16_gemm(x, W[n][0], W[n][1], out_dtype=torch.float32, workspace=ws)
+            return _sampled_columns_check(x, W[n][0], W[n][1], N, K, N + M, f"chain {n}", y=y)
+
+        qkv = lin("qkv", h)
+        att = renorm(qkv[:, :H])
+        o = lin("o", att)
+        h2 = renorm(h.float() + o)
+        gu = lin("gate_up", h2)
+        act = renorm(torch.nn.functional.silu(gu[:, :FF]) * gu[:, FF:])
+        d = lin("down", act)
+        assert torch.isfinite(d).all()
