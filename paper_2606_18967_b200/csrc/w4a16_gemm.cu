@@ -222,6 +222,11 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);
+  // Programmatic dependent launch: everything above touched no global memory, so it may overlap the tail of the
+  // previous kernel in the stream; from here on its results (X, the packed weights, the workspace) are needed.
+  // The next kernel may be scheduled as soon as SMs free up (it waits at its own griddepcontrol.wait).
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
   ER_TR(0);
 
   if (warp == 0) {
@@ -586,6 +591,7 @@ bool make_map_2d(CUtensorMap* map, CUtensorMapDataType dt, const void* base, uin
 unsigned long long* g_trace = nullptr;
 #endif
 int g_tune_dbg = 0;
+int g_tune_pdl = 1;          // programmatic dependent launch (key 3)
 int g_tune_force_ctas = 0;  // > 0: use this many CTAs (tests / sweeps); 0 = one per SM
 
 struct Plan {
@@ -624,8 +630,17 @@ int launch(const CUtensorMap& mx, const GemmParams& gp, const Plan& pl, cudaStre
                                      Cfg<MPAD>::kSmem));
     attr_set = true;
   }
-  w4a16_gemm_kernel<MPAD><<<pl.ctas, kThreads, Cfg<MPAD>::kSmem, stream>>>(mx, gp);
-  ER_CUDA_TRY(cudaGetLastError());
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)pl.ctas);
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = Cfg<MPAD>::kSmem;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = g_tune_pdl;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  ER_CUDA_TRY(cudaLaunchKernelEx(&cfg, w4a16_gemm_kernel<MPAD>, mx, gp));
   return ER_OK;
 }
 
@@ -639,7 +654,7 @@ int er_gemm_tuning(int key, int value) {
   if (key == 0 && (value == 1 || value == 2)) return ER_OK;
   if (key == 1 && value >= 0) { g_tune_force_ctas = value; return ER_OK; }
   if (key == 2 && value >= 0) { g_tune_dbg = value; return ER_OK; }
-  if (key == 3) return ER_OK;   // (retired knob)
+  if (key == 3 && (value == 0 || value == 1)) { g_tune_pdl = value; return ER_OK; }
   return ER_ERR_SHAPE;
 }
 
