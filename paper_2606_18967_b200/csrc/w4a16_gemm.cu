@@ -99,8 +99,15 @@ struct GemmParams {
     if ((id) < 8) tr_sum[(id)] += tr_now - tr_prev; \
     tr_prev = tr_now;                               \
   } while (0)
+#define ER_TR2(id)                                  \
+  do {                                              \
+    const unsigned tr_now = (unsigned)clock();      \
+    tr_sum2[(id)] += tr_now - tr_prev;              \
+    tr_prev = tr_now;                               \
+  } while (0)
 #else
 #define ER_TR(id) do {} while (0)
+#define ER_TR2(id) do {} while (0)
 #endif
 
 #define ER_TMEM_ST16(taddr, r, o)                                                                              \
@@ -202,6 +209,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   const int n_it = (int)(ge - gb);
 #ifdef ER_GEMM_TRACE
   unsigned tr_sum[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+  unsigned tr_sum2[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   unsigned tr_prev = (unsigned)clock();
 #endif
 
@@ -449,7 +457,9 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
         for (int m = 0; m < CW; ++m) mine[m * kTileN] = acc[m];
         named_bar_arrive(6, kThreads - kSetWarp0 * 32);
       } else {
+        ER_TR2(4);
         named_bar_sync(6, kThreads - kSetWarp0 * 32);
+        ER_TR2(5);
 #pragma unroll
         for (int j = 0; j < kSets - 1; ++j) {
           const float* theirs = red + (j * MPAD + half * CW) * kTileN + row;
@@ -481,8 +491,10 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
     // Ordering: partial stores (all threads) -> bar.sync -> the leader's acq_rel ticket (release is cumulative over
     // what the barrier made visible to the leader); last arriver: acq_rel ticket -> bar.sync -> ld.cg of the others'
     // partials.  No per-thread __threadfence on either side.
+    ER_TR2(0);
     if (set == 0 && (pend_tile[0] >= 0 || pend_tile[1] >= 0)) {
       named_bar_sync(7, kSetThreads);
+      ER_TR2(1);
       int c_lo[2] = {0, 0}, c_hi[2] = {-1, -1};
 #pragma unroll
       for (int k = 0; k < 2; ++k) {
@@ -506,7 +518,8 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
         }
       }
       named_bar_sync(7, kSetThreads);
-      constexpr int kChunk = CW <= 8 ? 4 : (CW <= 16 ? 2 : 1);   // contributors whose loads are in flight together
+      ER_TR2(2);
+      constexpr int kChunk = CW <= 8 ? 6 : (CW <= 16 ? 3 : 1);   // contributors whose loads are in flight together
 #pragma unroll
       for (int k = 0; k < 2; ++k) {
         if (pend_tile[k] < 0 || last_flag[k] == 0) continue;
@@ -534,6 +547,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
               if (c0 + j <= c_hi[k]) acc[m] += v[j][m];
         }
         store_tile(tile, acc);
+        ER_TR2(3);
       }
     }
   }
@@ -545,7 +559,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   if (warp == 1) tmem_dealloc<kTmemCols>(tmem);
 #ifdef ER_GEMM_TRACE
   if (p.trace && blockIdx.x == p.dbg_cta && lane == 0)
-    for (int i = 0; i < 8; ++i) p.trace[warp * 8 + i] = tr_sum[i];
+    for (int i = 0; i < 8; ++i) { p.trace[warp * 8 + i] = tr_sum[i]; p.trace[256 + warp * 8 + i] = tr_sum2[i]; }
 #endif
 }
 
