@@ -222,11 +222,9 @@ def reference_arm(args):
 # ------------------------------------------------------------------------------------------------------
 def product_arm(args):
     import torch
-    from paper_2606_18967_b200 import er, inputs as I
+    from paper_2606_18967_b200 import er, inputs as I, multi
 
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank, local_rank, world = multi.env_rank_world()
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the hot path has no CPU fallback (use --impl reference "
                          "for the oracle arm)")
@@ -396,10 +394,7 @@ def product_arm(args):
     torch.cuda.synchronize()
 
     stats = torch.cat([blk_ms, det.flatten(), torch.tensor([step_ms], dtype=torch.float64)])
-    if dist is not None:                                        # max over ranks, on the device
-        t = stats.to(dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        stats = t.cpu()
+    stats = multi.max_over_ranks(stats, dist, dev)              # max over ranks, on the device
     blk_ms, det, step_ms = stats[:4], stats[4:-1].reshape(len(Ms), len(linears)), float(stats[-1])
 
     peak, peak_src = hbm_peak()
@@ -426,7 +421,7 @@ def product_arm(args):
         if M <= 16:
             small_bytes, small_ms = small_bytes + tb, small_ms + tm
     blk_small_ms = float(blk_ms[1])                            # the M <= 16 block inside the timed step
-    value = small_bytes * world / blk_small_ms / 1e6           # GB/s, whole job
+    value = multi.whole_job_rate(small_bytes, world, blk_small_ms)   # GB/s, whole job
     achieved = k16_bytes / blk_small_ms / 1e6
     k16_ms = blk_small_ms
     verify_bytes = B * (2 * G + 1) * V * 2.0
