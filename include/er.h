@@ -98,9 +98,14 @@ int er_quantize_pack(const void* w_bf16, int64_t N, int64_t K, int64_t ldw_elems
  *   y        [M][N] of y_dtype (ER_BF16: fp32 accumulator rounded RNE; ER_F32: the accumulator itself),
  *            row stride ldy_elems; rows >= M are never written
  *   workspace  caller-provided, >= er_gemm_workspace_bytes(M,N,K), 16-byte aligned, counters zeroed once
- * Arithmetic: codes are widened exactly to bf16, contracted with X on the tensor cores with fp32
- * accumulation per 128-k group, each group's partial sum multiplied by its fp32 scale and added in fp32
- * (no rounding of q*s), split-K partials reduced in ascending split order. */
+ *            (N/128) * (K/128) * ceil(M / 64) must stay below 2^31 (else ER_ERR_SHAPE)
+ * Arithmetic: stored nibbles u = q + 8 are widened exactly to bf16 (as 128 + u), contracted with X on the
+ * tensor cores with fp32 accumulation per 128-k group; the same accumulator receives -136 * sum_k x[m][k]
+ * (the offset, through a constant operand tile), so it holds sum_k x * q up to fp32 rounding; each group's
+ * sum is multiplied by its fp32 scale and added in fp32 (no rounding of q*s); split-K partials are reduced
+ * in ascending CTA order (deterministic).
+ * Launch: one persistent kernel, launched with programmatic stream serialization; it touches no global
+ * memory before griddepcontrol.wait, so ordering against earlier work in the stream is the usual one. */
 int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems,
                   const void* qweight, const void* scales, int64_t N, int group,
                   void* y, int64_t ldy_elems, int y_dtype,

@@ -8,9 +8,10 @@
 // owns a contiguous range of 2048-token tiles of the vocabulary; rows are streamed with 128-bit loads (8
 // consecutive elements per thread).  Per-row softmax normalisers and residual masses are reduced inside the
 // CTA, exchanged through distributed shared memory and combined in rank order by every CTA, so all CTAs of
-// a cluster take the same decisions.  The accept scan is lazy: position i's normalisers are only computed if
-// positions < i were all accepted, so a sequence rejected at position n reads 2 (n + 1) rows instead of
-// 2 gamma + 1.  The residual draw is a multi-level inverse CDF: per-warp segment sums (256 consecutive
+// a cluster take the same decisions.  The statistics of all gamma + 1 positions are computed in ONE sweep with
+// one cluster exchange (a lazy scan, stopping at the first rejection, reads less when acceptance is low but
+// pays a cluster barrier and a DRAM round trip per position; with the paper's acceptance of ~0.98 every row is
+// needed anyway).  The residual draw is a multi-level inverse CDF: per-warp segment sums (256 consecutive
 // tokens) -> per-CTA totals, exchanged -> the CTA whose range holds the threshold does an fp64 prefix over
 // its segments and a warp scan inside the one segment that contains the threshold.
 #include <cooperative_groups.h>
@@ -89,6 +90,15 @@ __device__ __forceinline__ void load8(const T* row, int v0, int V, bool vec, flo
   Load8<T>::expand(Load8<T>::load(row, v0, V, vec, fill), f);
 }
 
+// 2^x by the special-function unit alone (relative error about 2^-22; no range-reduction code around it)
+__device__ __forceinline__ float ex2_fast(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 __device__ __forceinline__ float warp_max(float x) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) x = fmaxf(x, __shfl_xor_sync(0xffffffffu, x, o));
@@ -106,12 +116,11 @@ struct RowStats {
 };
 
 struct Shared {
-  float4 xstats[2][kMaxCluster];   // [parity][rank]: (max_t, sum_t, max_d, sum_d) of every CTA's vocabulary range
   double xmass[2][kMaxCluster];    // [parity][rank]: residual mass of every CTA's range
-  float red_a[kWarps];
-  float red_b[kWarps];
+  float4 wstat[17][kWarps];        // [position][warp]: per-warp (max_t, sum_t, max_d, sum_d) of this CTA's range
+  float4 xall[kMaxCluster][17];    // [rank][position]: per-CTA statistics of every CTA of the cluster
+  float4 stat[17];                 // [position]: (max_t, 1/sum_t, max_d, 1/sum_d) over the whole vocabulary
   float px[16], qx[16], ua[16];    // target / draft value at the drafted token and the uniform, per position
-  float bc[4];
   int seg;
   int token;
   int flag;
@@ -124,11 +133,11 @@ struct ClusterCtx {
   int xpar;            // parity of the next exchange buffer
 };
 
-// Softmax normalisers of one target row and (optionally) one draft row in a single pass over this CTA's tile
-// range (online max/sum), then combined over the cluster in rank order: identical in every CTA.
+// Softmax statistics (online max / sum of exponentials) of one target row and (optionally) one draft row over
+// this CTA's tile range, reduced to one entry per warp in sh.wstat[pos].
 template <typename T>
-__device__ void row_stats(const T* trow, const T* drow, int V, bool vec, float scale, Shared& sh, ClusterCtx& cx,
-                          RowStats& st, RowStats& sd) {
+__device__ void row_stats(const T* trow, const T* drow, const T* next_t, const T* next_d, int V, bool vec, float scale,
+                          Shared& sh, ClusterCtx& cx, int pos) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   float mt = kNegInf, st_ = 0.f, md = kNegInf, sd_ = 0.f;
   constexpr int NB = Load8<T>::kBatch;
@@ -140,6 +149,10 @@ __device__ void row_stats(const T* trow, const T* drow, int V, bool vec, float s
       if (t0 + j < cx.tile_hi && v0 < V) {
         rt[j] = Load8<T>::load(trow, v0, V, vec, kNegInf);
         if (drow) rd[j] = Load8<T>::load(drow, v0, V, vec, kNegInf);
+        // the same tile of the NEXT position goes to L2 now: one position (~80 KB per CTA) of run-ahead, so
+        // only the very first batch of the sweep pays a DRAM round trip per warp
+        if (next_t) prefetch_l2(next_t + v0);
+        if (next_d) prefetch_l2(next_d + v0);
       }
     }
 #pragma unroll
@@ -152,56 +165,66 @@ __device__ void row_stats(const T* trow, const T* drow, int V, bool vec, float s
 #pragma unroll
         for (int i = 1; i < 8; ++i) cm = fmaxf(cm, f[i]);
         if (cm > mt) { st_ *= exp2f((mt - cm) * scale); mt = cm; }
+        const float nt = -mt * scale;
 #pragma unroll
-        for (int i = 0; i < 8; ++i) st_ += exp2f((f[i] - mt) * scale);
+        for (int i = 0; i < 8; ++i) st_ += ex2_fast(fmaf(f[i], scale, nt));
         if (drow) {
           Load8<T>::expand(rd[j], f);
           cm = f[0];
 #pragma unroll
           for (int i = 1; i < 8; ++i) cm = fmaxf(cm, f[i]);
           if (cm > md) { sd_ *= exp2f((md - cm) * scale); md = cm; }
+          const float nd = -md * scale;
 #pragma unroll
-          for (int i = 0; i < 8; ++i) sd_ += exp2f((f[i] - md) * scale);
+          for (int i = 0; i < 8; ++i) sd_ += ex2_fast(fmaf(f[i], scale, nd));
         }
       }
     }
   }
-  // CTA max
-  float wm_t = warp_max(mt), wm_d = warp_max(md);
-  if (lane == 0) { sh.red_a[warp] = wm_t; sh.red_b[warp] = wm_d; }
-  __syncthreads();
-  float bm_t = lane < kWarps ? sh.red_a[lane] : kNegInf, bm_d = lane < kWarps ? sh.red_b[lane] : kNegInf;
-  bm_t = warp_max(bm_t); bm_d = warp_max(bm_d);
-  __syncthreads();
-  // CTA sum of rescaled partial sums
-  st_ = (mt > kNegInf) ? st_ * exp2f((mt - bm_t) * scale) : 0.f;
-  sd_ = (md > kNegInf) ? sd_ * exp2f((md - bm_d) * scale) : 0.f;
-  float ws_t = warp_sum(st_), ws_d = warp_sum(sd_);
-  if (lane == 0) { sh.red_a[warp] = ws_t; sh.red_b[warp] = ws_d; }
-  __syncthreads();
-  float bs_t = warp_sum(lane < kWarps ? sh.red_a[lane] : 0.f), bs_d = warp_sum(lane < kWarps ? sh.red_b[lane] : 0.f);
-  // cluster: every CTA publishes its (max, sum) pair to all CTAs, then all combine in rank order
+  // warp level only (no CTA barrier per position): max, then the sum of the rescaled partial sums
+  const float wm_t = warp_max(mt), wm_d = warp_max(md);
+  st_ = (mt > kNegInf) ? st_ * exp2f((mt - wm_t) * scale) : 0.f;
+  sd_ = (md > kNegInf) ? sd_ * exp2f((md - wm_d) * scale) : 0.f;
+  const float ws_t = warp_sum(st_), ws_d = warp_sum(sd_);
+  if (lane == 0) sh.wstat[pos][warp] = make_float4(wm_t, ws_t, wm_d, ws_d);
+}
+
+// (max, sum) pairs a and b of two disjoint parts of a row -> the pair of their union
+__device__ __forceinline__ void merge_stat(float& m, float& s, float m2, float s2, float scale) {
+  const float mm = fmaxf(m, m2);
+  const float a = (m > kNegInf) ? s * exp2f((m - mm) * scale) : 0.f;
+  const float b = (m2 > kNegInf) ? s2 * exp2f((m2 - mm) * scale) : 0.f;
+  m = mm;
+  s = a + b;
+}
+
+// After row_stats of positions 0..npos-1: combine warps (in order), exchange over the cluster through
+// distributed shared memory, combine ranks (in order).  Every CTA ends with the same sh.stat[].
+__device__ void combine_stats(int npos, float scale, Shared& sh, ClusterCtx& cx) {
+  const int tid = threadIdx.x;
   cg::cluster_group cluster = cg::this_cluster();
-  const int par = cx.xpar;
-  cx.xpar ^= 1;
-  if (tid < cx.size) {
-    float4* dst = cluster.map_shared_rank(&sh.xstats[par][cx.rank], tid);
-    *dst = make_float4(bm_t, bs_t, bm_d, bs_d);
+  __syncthreads();
+  if (tid < npos) {
+    float mt = kNegInf, st = 0.f, md = kNegInf, sd = 0.f;
+    for (int w = 0; w < kWarps; ++w) {
+      const float4 v = sh.wstat[tid][w];
+      merge_stat(mt, st, v.x, v.y, scale);
+      merge_stat(md, sd, v.z, v.w, scale);
+    }
+    const float4 mine = make_float4(mt, st, md, sd);
+    for (int c = 0; c < cx.size; ++c) *cluster.map_shared_rank(&sh.xall[cx.rank][tid], c) = mine;
   }
   cluster.sync();
-  float gm_t = kNegInf, gm_d = kNegInf;
-  for (int c = 0; c < cx.size; ++c) {
-    gm_t = fmaxf(gm_t, sh.xstats[par][c].x);
-    gm_d = fmaxf(gm_d, sh.xstats[par][c].z);
+  if (tid < npos) {
+    float mt = kNegInf, st = 0.f, md = kNegInf, sd = 0.f;
+    for (int c = 0; c < cx.size; ++c) {
+      const float4 v = sh.xall[c][tid];
+      merge_stat(mt, st, v.x, v.y, scale);
+      merge_stat(md, sd, v.z, v.w, scale);
+    }
+    sh.stat[tid] = make_float4(mt, __fdiv_rn(1.0f, st), md, sd > 0.f ? __fdiv_rn(1.0f, sd) : 0.f);
   }
-  float gs_t = 0.f, gs_d = 0.f;
-  for (int c = 0; c < cx.size; ++c) {
-    const float4 v = sh.xstats[par][c];
-    if (v.x > kNegInf) gs_t += v.y * exp2f((v.x - gm_t) * scale);
-    if (v.z > kNegInf) gs_d += v.w * exp2f((v.z - gm_d) * scale);
-  }
-  st.max = gm_t; st.inv_sum = __fdiv_rn(1.0f, gs_t);
-  sd.max = gm_d; sd.inv_sum = drow ? __fdiv_rn(1.0f, gs_d) : 0.f;
+  __syncthreads();
 }
 
 // The 8 residual weights of one thread chunk from its raw loads.  use_q == false: w = p (bonus token /
@@ -214,14 +237,18 @@ __device__ __forceinline__ void weights8_raw(const typename Load8<T>::Raw& rp, c
   Load8<T>::expand(rp, p);
   if (kLogits) {
 #pragma unroll
-    for (int i = 0; i < 8; ++i) p[i] = exp2f((p[i] - st.max) * scale) * st.inv_sum;
+    const float nt = -st.max * scale;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) p[i] = ex2_fast(fmaf(p[i], scale, nt)) * st.inv_sum;
   }
   if (use_q) {
     float q[8];
     Load8<T>::expand(rq, q);
     if (kLogits) {
 #pragma unroll
-      for (int i = 0; i < 8; ++i) q[i] = exp2f((q[i] - sd.max) * scale) * sd.inv_sum;
+      const float nd = -sd.max * scale;
+#pragma unroll
+      for (int i = 0; i < 8; ++i) q[i] = ex2_fast(fmaf(q[i], scale, nd)) * sd.inv_sum;
     }
 #pragma unroll
     for (int i = 0; i < 8; ++i) w[i] = fmaxf(0.f, p[i] - q[i]);
@@ -281,8 +308,10 @@ __device__ int draw_token(const T* trow, const T* drow, int V, bool vec, float s
   cx.xpar ^= 1;
   const int nseg = ntile * kWarps;
   if (warp == 0) {
-    double mine = 0.0;
-    for (int i = 0; i < nseg; ++i) mine += (double)seg_sums[i];   // every lane: the same sequential sum
+    double mine = 0.0;                       // lane-strided partial sums, then a butterfly: the same value in
+    for (int i = lane; i < nseg; i += 32) mine += (double)seg_sums[i];   // every lane, in a fixed order
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mine += __shfl_xor_sync(0xffffffffu, mine, o);
     if (lane < cx.size) *cluster.map_shared_rank(&sh.xmass[par][cx.rank], lane) = mine;
   }
   cluster.sync();
@@ -309,16 +338,19 @@ __device__ int draw_token(const T* trow, const T* drow, int V, bool vec, float s
   if (tid == 0) {
     const double thr_cta = thr - before;
     double c = 0.0;
-    int seg = nseg - 1;
+    int seg = -1;
     for (int i = 0; i < nseg; ++i) {
       const double nc = c + (double)seg_sums[i];
       if (nc > thr_cta) { seg = i; break; }
       c = nc;
     }
-    while (seg > 0 && !(seg_sums[seg] > 0.f)) --seg;
-    double excl = 0.0;
-    for (int i = 0; i < seg; ++i) excl += (double)seg_sums[i];
-    sh.thr_local = thr_cta - excl;
+    if (seg < 0) {      // rounding left no segment (the rank was chosen from a differently ordered sum): take
+      seg = nseg - 1;   // the last segment with mass and recompute its exclusive prefix
+      while (seg > 0 && !(seg_sums[seg] > 0.f)) --seg;
+      c = 0.0;
+      for (int i = 0; i < seg; ++i) c += (double)seg_sums[i];
+    }
+    sh.thr_local = thr_cta - c;
     sh.seg = seg;
     sh.token = -1;
   }
@@ -398,29 +430,43 @@ spec_verify_kernel(const T* __restrict__ target, const T* __restrict__ draft, fl
   }
   __syncthreads();
 
-  RowStats st{0.f, 1.f}, sd{0.f, 1.f};
-  int n = 0;
-  for (; n < gamma; ++n) {
-    const T* trow = tgt + (size_t)n * V;
-    const T* drow = drf + (size_t)n * V;
-    if (kLogits) row_stats<T>(trow, drow, V, vec, scale, sh, cx, st, sd);
-    if (tid == 0) {            // every CTA of the cluster takes the same decision from the same numbers
-      float p = sh.px[n], q = sh.qx[n];
-      if (kLogits) {
-        p = exp2f((p - st.max) * scale) * st.inv_sum;
-        q = exp2f((q - sd.max) * scale) * sd.inv_sum;
-      }
-      const float lhs = __fmul_rn(sh.ua[n], q);
-      sh.flag = (lhs < p) ? 1 : 0;
+  // Statistics of ALL gamma + 1 positions in one sweep and one cluster exchange.  (A lazy scan would skip the rows
+  // behind the first rejection, but costs a cluster barrier and a DRAM round trip per position; in the paper's
+  // regime nearly every drafted token is accepted, so those rows are needed anyway.)
+  if (kLogits) {
+    for (int t = cx.tile_lo; t < cx.tile_hi; ++t) {     // position 0: everything behind the first batch to L2
+      const int v0 = t * kTile + tid * kPerThread;
+      if (v0 < V) { prefetch_l2(tgt + v0); prefetch_l2(drf + v0); }
     }
-    __syncthreads();
-    const int acc = sh.flag;
-    __syncthreads();
-    if (!acc) break;
+    for (int i = 0; i <= gamma; ++i)
+      row_stats<T>(tgt + (size_t)i * V, i < gamma ? drf + (size_t)i * V : nullptr,
+                   i < gamma ? tgt + (size_t)(i + 1) * V : nullptr, i + 1 < gamma ? drf + (size_t)(i + 1) * V : nullptr,
+                   V, vec, scale, sh, cx, i);
+    combine_stats(gamma + 1, scale, sh, cx);
+  }
+  if (tid == 0) {              // every CTA of the cluster takes the same decisions from the same numbers
+    int k = 0;
+    for (; k < gamma; ++k) {
+      float p = sh.px[k], q = sh.qx[k];
+      if (kLogits) {
+        const float4 v = sh.stat[k];
+        p = exp2f((p - v.x) * scale) * v.y;
+        q = exp2f((q - v.z) * scale) * v.w;
+      }
+      const float lhs = __fmul_rn(sh.ua[k], q);
+      if (!(lhs < p)) break;
+    }
+    sh.flag = k;
+  }
+  __syncthreads();
+  const int n = sh.flag;
+  RowStats st{0.f, 1.f}, sd{0.f, 1.f};
+  if (kLogits) {
+    const float4 v = sh.stat[n];
+    st.max = v.x; st.inv_sum = v.y; sd.max = v.z; sd.inv_sum = v.w;
   }
   const T* trow = tgt + (size_t)n * V;
   const T* drow = (n < gamma) ? drf + (size_t)n * V : nullptr;
-  if (n == gamma && kLogits) row_stats<T>(trow, nullptr, V, vec, scale, sh, cx, st, sd);
   const float r = u_sample[b];
   int tok = draw_token<T, kLogits>(trow, drow, V, vec, scale, st, sd, n < gamma, r, sh, cx, seg_sums);
   if (tok == -1) tok = draw_token<T, kLogits>(trow, nullptr, V, vec, scale, st, sd, false, r, sh, cx, seg_sums);
@@ -456,7 +502,15 @@ int launch_verify(int cluster_size, size_t smem, cudaStream_t s, const T* target
   return ER_OK;
 }
 
+int g_force_cluster = 0;   // sweeps only (er_verify_tuning): 0 = automatic
+
 }  // namespace
+
+extern "C" int er_verify_tuning(int cluster) {
+  if (cluster != 0 && cluster != 1 && cluster != 2 && cluster != 4 && cluster != 8) return ER_ERR_SHAPE;
+  g_force_cluster = cluster;
+  return ER_OK;
+}
 
 extern "C" int er_spec_verify(const void* target, const void* draft, int in_dtype, int inputs_are_logits,
                               float temperature, const int32_t* draft_tokens, const float* u_accept,
@@ -472,7 +526,8 @@ extern "C" int er_spec_verify(const void* target, const void* draft, int in_dtyp
   int st = er::check_arch();
   if (st != ER_OK) return st;
   const int tiles = (V + kTile - 1) / kTile;
-  const int cluster = tiles >= 8 ? 8 : (tiles >= 4 ? 4 : (tiles >= 2 ? 2 : 1));   // CTAs per sequence
+  int cluster = tiles >= 8 ? 8 : (tiles >= 4 ? 4 : (tiles >= 2 ? 2 : 1));   // CTAs per sequence
+  if (g_force_cluster > 0 && g_force_cluster <= cluster) cluster = g_force_cluster;
   const int per = (tiles + cluster - 1) / cluster;
   const size_t smem = (size_t)per * kWarps * sizeof(float);
   const float scale = (float)(1.4426950408889634 / (double)temperature);
