@@ -217,3 +217,25 @@ def test_config2_layer_chain_teacher_forced_shrinking_batch():
         act = renorm(torch.nn.functional.silu(gu[:, :FF]) * gu[:, FF:])
         d = lin("down", act)
         assert torch.isfinite(d).all()
+
+
+def test_programmatic_dependent_launch_does_not_change_results():
+    # er_w4a16_gemm is launched with programmatic stream serialization; back-to-back calls that depend on each other
+    # (same Y / workspace, chained X) must give the same bits with it switched off
+    N, K, M = 3584, 3584, 8
+    w = I.weight_bf16(N, K, I.seed_of("pdl", "w"), device=DEV)
+    qw, sc = er.quantize_pack(w)
+    x0 = I.activation_bf16(M, K, I.seed_of("pdl", "x"), device=DEV)
+    ws = er.gemm_workspace(M, N, K, DEV)
+    lib = er.load()
+    outs = []
+    for pdl in (1, 0):
+        assert lib.er_gemm_tuning(3, pdl) == 0
+        x = x0
+        for _ in range(4):          # y feeds the next call: a chain of dependent launches
+            y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.bfloat16, workspace=ws)
+            x = (y.float() / y.float().pow(2).mean().sqrt()).to(torch.bfloat16)
+        torch.cuda.synchronize()
+        outs.append(y.clone())
+    lib.er_gemm_tuning(3, 1)
+    assert torch.equal(outs[0], outs[1])

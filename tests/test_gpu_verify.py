@@ -125,3 +125,29 @@ def test_deterministic():
     a1, o1 = er.spec_verify(t, d, toks, ua, us, True)
     a2, o2 = er.spec_verify(t, d, toks, ua, us, True)
     assert torch.equal(a1, a2) and torch.equal(o1, o2)
+
+
+def test_max_gamma_and_high_acceptance():
+    # gamma = 16 (the maximum), draft close to target: most tokens are accepted, several sequences reach the bonus
+    # position (the paper's regime); vocabulary not a multiple of the tile
+    B, gamma, V = 3, 16, 50001
+    lt, ld = I.verify_logits_f32(B, gamma, V, 901, draft_noise=0.05)
+    toks = I.sample_draft_tokens(_softmax(ld), 902)
+    acc, out, _ = _run_and_check(lt, ld, toks, I.uniforms((B, gamma), 903), I.uniforms((B,), 904), True, torch.float32)
+    assert acc.max() >= gamma // 2
+
+
+@pytest.mark.parametrize("cluster", [1, 2, 4, 8])
+def test_every_cluster_size_gives_the_same_tokens(cluster):
+    # the per-sequence work may be split over 1-8 CTAs; decisions and accepted prefixes must not depend on the
+    # split (the drawn token may differ only inside the V10 window, which _run_and_check enforces)
+    B, gamma, V = 6, 4, 152064
+    lt, ld = I.verify_logits_f32(B, gamma, V, 911, draft_noise=0.5)
+    toks = I.sample_draft_tokens(_softmax(ld), 912)
+    ua, us = I.uniforms((B, gamma), 913), I.uniforms((B,), 914)
+    lib = er.load()
+    assert lib.er_verify_tuning(cluster) == 0
+    try:
+        _run_and_check(lt, ld, toks, ua, us, True, torch.float32)
+    finally:
+        lib.er_verify_tuning(0)
