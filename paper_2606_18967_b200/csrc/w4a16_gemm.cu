@@ -264,47 +264,50 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
       }
       if (++s == S) { s = 0; ph ^= 1; }
     }
-  } else if (warp <= kBuf) {
+  } else if (warp <= 2) {
     // ===================== MMA issuers (warp-uniform; one elected lane issues) =====================
-    // With two buffers per set, warp 1 takes the even groups of the range and warp 2 the odd ones (they sit on
-    // different SM sub-partitions, whose issue slots the worker warps keep busy: one issuer alone is too slow).
-    // A given (set, buffer) pair is then always served by the same issuer, which therefore sees every phase
-    // of its a_full barrier; with one buffer per set that would not hold, so a single warp issues everything.
+    // Two issuers, on different SM sub-partitions (the worker warps keep the issue slots busy: one issuer alone is
+    // too slow).  An a_full barrier must always be served by the same issuer, which then sees every one of its
+    // phases: with two buffers per set warp 1 takes the even groups of the range and warp 2 the odd ones (a
+    // (set, buffer) pair has a fixed group parity); with one buffer per set warp 1 serves sets 0 and 2, warp 2
+    // serves set 1.
     constexpr uint32_t idesc = idesc_bf16_m128(MPAD);
-    int s = warp - 1;
+    int s = 0, set = 0, i = 0;           // stage, set and the set's group count of group `it`
     uint32_t ph = 0;                     // parity of full[s] (streaming-only mode)
-    for (int it = warp - 1; it < n_it; it += kBuf) {
-      if (p.dbg & 64) {
-        mbar_wait(&full[s], ph);
-        if (elect_one()) mbar_arrive(&empty[s]);
-      } else {
-        const int i = it / kSets, set = it - i * kSets;   // the set's i-th group
-        const int bi = set * kBuf + (i % kBuf);
-        mbar_wait(&a_full[bi], (i / kBuf) & 1);            // implies full[s] (the set waited for it)
-        ER_TR(1);
-        tc_fence_after();
-        if (elect_one()) {
-          const uint32_t xbase = smem_u32(smem + s * C::kStageBytes + kWBytes);
-          const uint32_t d_t = tmem + C::kTmemD + bi * MPAD;
-          const uint32_t a_t = tmem + kTmemA + bi * 64;
+    for (int it = 0; it < n_it; ++it) {
+      const bool mine = (kBuf == 2) ? ((it & 1) == warp - 1) : ((set == 1) == (warp == 2));
+      if (mine) {
+        if (p.dbg & 64) {
+          mbar_wait(&full[s], ph);
+          if (elect_one()) mbar_arrive(&empty[s]);
+        } else {
+          const int bi = set * kBuf + (i % kBuf);
+          mbar_wait(&a_full[bi], (i / kBuf) & 1);            // implies full[s] (the set waited for it)
+          ER_TR(1);
+          tc_fence_after();
+          if (elect_one()) {
+            const uint32_t xbase = smem_u32(smem + s * C::kStageBytes + kWBytes);
+            const uint32_t d_t = tmem + C::kTmemD + bi * MPAD;
+            const uint32_t a_t = tmem + kTmemA + bi * 64;
 #pragma unroll
-          for (int kk = 0; kk < 8; ++kk) {
-            const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
-            mma_ts_f16(d_t, a_t + kk * 8, bdesc, idesc, kk > 0 ? 1u : 0u);
-          }
+            for (int kk = 0; kk < 8; ++kk) {
+              const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
+              mma_ts_f16(d_t, a_t + kk * 8, bdesc, idesc, kk > 0 ? 1u : 0u);
+            }
 #pragma unroll
-          for (int kk = 0; kk < 8; ++kk) {   // - 136 * sum_k x[m][k]: the offset of the stored nibble
-            const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
-            mma_ts_f16(d_t, tmem + C::kTmemConst + set * 8, bdesc, idesc, 1u);
+            for (int kk = 0; kk < 8; ++kk) {   // - 136 * sum_k x[m][k]: the offset of the stored nibble
+              const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
+              mma_ts_f16(d_t, tmem + C::kTmemConst + set * 8, bdesc, idesc, 1u);
+            }
+            tc_commit(&done[bi]);
+            tc_commit(&empty[s]);
           }
-          tc_commit(&done[bi]);
-          tc_commit(&empty[s]);
         }
+        __syncwarp();
+        ER_TR(2);
       }
-      __syncwarp();
-      ER_TR(2);
-      s += kBuf;
-      if (s >= S) { s -= S; ph ^= 1; }
+      if (++s == S) { s = 0; ph ^= 1; }
+      if (++set == kSets) { set = 0; ++i; }
     }
   } else if (warp >= kSetWarp0) {
     // ===================== worker sets: convert, scale-accumulate, output =====================
