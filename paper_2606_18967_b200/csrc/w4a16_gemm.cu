@@ -58,6 +58,7 @@ struct Cfg {
   static constexpr int kSmem = kStages * kStageBytes + kFixed;
   static constexpr uint32_t kTxBytes = kWBytes + kXBytes + kScaleBytes;
   static constexpr int kCW = MPAD / 2;                     // accumulator columns per thread (half of the batch rows)
+  static constexpr bool kSubInWorkers = (MPAD > 32);      // see dequant_word
   static constexpr bool kEpiFirst = (MPAD > 32);           // register pressure: read back before converting
   // TMEM: every set owns kBuf (A operand, accumulator) pairs.  Two pairs (M <= 16, where the columns allow it)
   // let a set convert group i + 1 while the MMAs of group i are still in flight.
@@ -146,9 +147,16 @@ __device__ __forceinline__ uint32_t lop3_and_or(uint32_t a, uint32_t mask, uint3
 // removed here (one packed fma per pair would cost as many issue cycles again) but folded into the
 // contraction: eight more MMAs per group with a constant A tile of -136 add -136 * sum_k x to the accumulator.
 // (An fp16 A operand would need 5 logic ops, but tcgen05.mma.kind::f16 faults on fp16 A x bf16 B.)
+// kSub: remove the 136 here with one packed fma per pair (used where the tensor pipe, not the logic pipe, is the
+// busier one: at N = 64 the eight constant-tile MMAs per group cost more than the subtracts).
+template <bool kSub>
 __device__ __forceinline__ void dequant_word(uint32_t w, uint32_t* a) {
 #pragma unroll
-  for (int t = 0; t < 4; ++t) a[t] = lop3_and_or(w >> (4 * t), 0x000F000Fu, 0x43004300u);
+  for (int t = 0; t < 4; ++t) {
+    const uint32_t v = lop3_and_or(w >> (4 * t), 0x000F000Fu, 0x43004300u);
+    if (kSub) asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(a[t]) : "r"(v), "r"(0x3F803F80u), "r"(0xC308C308u));
+    else a[t] = v;
+  }
 }
 
 __device__ __forceinline__ uint4 lds128(uint32_t saddr) {
@@ -295,7 +303,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
               mma_ts_f16(d_t, a_t + kk * 8, bdesc, idesc, kk > 0 ? 1u : 0u);
             }
 #pragma unroll
-            for (int kk = 0; kk < 8; ++kk) {   // - 136 * sum_k x[m][k]: the offset of the stored nibble
+            for (int kk = 0; kk < (C::kSubInWorkers ? 0 : 8); ++kk) {   // - 136 * sum_k x[m][k]: the stored nibble's offset
               const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
               mma_ts_f16(d_t, tmem + C::kTmemConst + set * 8, bdesc, idesc, 1u);
             }
@@ -416,14 +424,14 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
           const uint4 pk1 = lds128(st + w_addr1);
           const uint32_t sc16 = lds_u16(st + sc_addr);
           uint32_t a[32];
-          dequant_word(pk0.x, a + 0);
-          dequant_word(pk0.y, a + 4);
-          dequant_word(pk0.z, a + 8);
-          dequant_word(pk0.w, a + 12);
-          dequant_word(pk1.x, a + 16);
-          dequant_word(pk1.y, a + 20);
-          dequant_word(pk1.z, a + 24);
-          dequant_word(pk1.w, a + 28);
+          dequant_word<C::kSubInWorkers>(pk0.x, a + 0);
+          dequant_word<C::kSubInWorkers>(pk0.y, a + 4);
+          dequant_word<C::kSubInWorkers>(pk0.z, a + 8);
+          dequant_word<C::kSubInWorkers>(pk0.w, a + 12);
+          dequant_word<C::kSubInWorkers>(pk1.x, a + 16);
+          dequant_word<C::kSubInWorkers>(pk1.y, a + 20);
+          dequant_word<C::kSubInWorkers>(pk1.z, a + 24);
+          dequant_word<C::kSubInWorkers>(pk1.w, a + 28);
           ER_TR(2);
           // the set's previous group: its MMAs had this whole conversion to finish; after this the A buffer
           // (read by those MMAs) and the accumulator are free again
