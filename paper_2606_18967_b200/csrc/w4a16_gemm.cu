@@ -76,6 +76,7 @@ struct GemmParams {
   int unit_groups;     // groups per scheduling unit: 1 (stream-K) or G (whole tiles)
   int units;           // tiles * G / unit_groups (< 2^31, checked on the host)
   int uq, ur;          // units / CTAs and units % CTAs: CTA c owns units [c*uq + min(c, ur), ...)
+  int split;           // > 0: tile split (see range_begin); uq = groups per tile
   int y_f32;
   int64_t ldy;
   void* y;
@@ -180,11 +181,26 @@ __device__ __forceinline__ void sts_f32(uint32_t saddr, float v) {
 
 __device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
-// first unit of CTA c when the units are dealt to the CTAs as contiguous, balanced ranges (the first `ur` CTAs
-// get uq + 1 units, the others uq); 32-bit arithmetic only
-__device__ __forceinline__ int range_begin(int uq, int ur, int c) { return c * uq + min(c, ur); }
+// Work partition (32-bit arithmetic only).  split == 0 ("stream-K"): the units are dealt to the CTAs as contiguous,
+// balanced ranges -- the first `ur` CTAs get uq + 1 units, the others uq.  split == k > 0 ("tile split", chosen when
+// tiles * k CTAs fit the SMs): CTA c owns part c % k of tile c / k, so no CTA straddles two tiles (one segment, one
+// partial sum, one ticket per CTA) -- only for unit_groups == 1; uq then holds the groups per tile.
+__device__ __forceinline__ int range_begin(int uq, int ur, int split, int c) {
+  if (split > 0) {
+    const int t = c / split, j = c - t * split;
+    return t * uq + (j * uq) / split;
+  }
+  return c * uq + min(c, ur);
+}
 // the CTA whose range contains unit u
-__device__ __forceinline__ int owner_of(int uq, int ur, int u) {
+__device__ __forceinline__ int owner_of(int uq, int ur, int split, int u) {
+  if (split > 0) {
+    const int t = u / uq, g = u - t * uq;
+    int j = (g * split) / uq;                        // close; fix up against the exact boundaries
+    while (j + 1 < split && ((j + 1) * uq) / split <= g) ++j;
+    while (j > 0 && (j * uq) / split > g) --j;
+    return t * split + j;
+  }
   const int big = ur * (uq + 1);
   return u < big ? u / (uq + 1) : ur + (u - big) / uq;
 }
@@ -212,8 +228,8 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   const int lane = threadIdx.x & 31;
   const int P = gridDim.x, cta = blockIdx.x;
   const int ug = p.unit_groups;
-  const int gb = range_begin(p.uq, p.ur, cta) * ug;        // first global group index of this CTA
-  const int ge = range_begin(p.uq, p.ur, cta + 1) * ug;
+  const int gb = range_begin(p.uq, p.ur, p.split, cta) * ug;        // first global group index of this CTA
+  const int ge = range_begin(p.uq, p.ur, p.split, cta + 1) * ug;
   const int n_it = (int)(ge - gb);
 #ifdef ER_GEMM_TRACE
   unsigned tr_sum[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -512,8 +528,8 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
         if (pend_tile[k] < 0) continue;
         const int u_first = (pend_tile[k] * p.G) / ug;
         const int u_last = ((pend_tile[k] + 1) * p.G - 1) / ug;
-        c_lo[k] = owner_of(p.uq, p.ur, u_first);
-        c_hi[k] = owner_of(p.uq, p.ur, u_last);
+        c_lo[k] = owner_of(p.uq, p.ur, p.split, u_first);
+        c_hi[k] = owner_of(p.uq, p.ur, p.split, u_last);
       }
       if (leader) {
         int old[2] = {0, 0};
@@ -545,7 +561,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
           for (int j = 0; j < kChunk; ++j) {
             const int c = min(c0 + j, c_hi[k]);
             // CTA c's piece of this tile is its first segment iff its range starts inside the tile
-            const int cb = range_begin(p.uq, p.ur, c) * ug;
+            const int cb = range_begin(p.uq, p.ur, p.split, c) * ug;
             const int which = (cb >= tile * p.G) ? 0 : 1;
             const float* src = p.partials + ((size_t)c * 2 + which) * (MPAD * kTileN) + half * CW * kTileN;
 #pragma unroll
@@ -617,10 +633,11 @@ unsigned long long* g_trace = nullptr;
 #endif
 int g_tune_dbg = 0;
 int g_tune_pdl = 1;          // programmatic dependent launch (key 3)
+int g_tune_split = 1;        // tile split where it applies (key 4)
 int g_tune_force_ctas = 0;  // > 0: use this many CTAs (tests / sweeps); 0 = one per SM
 
 struct Plan {
-  int mpad, mchunks, ntiles, tiles, G, unit_groups, ctas;
+  int mpad, mchunks, ntiles, tiles, G, unit_groups, ctas, split;
   long long units;
 };
 
@@ -640,6 +657,15 @@ Plan make_plan(int64_t M, int64_t N, int64_t K) {
   if (g_tune_force_ctas > 0 && g_tune_force_ctas < ctas) ctas = g_tune_force_ctas;
   if ((long long)ctas > pl.units) ctas = (int)pl.units;
   pl.ctas = ctas;
+  // tile split: when k >= 2 parts per tile fill at least 90 % of the CTAs, no CTA has to straddle two tiles
+  pl.split = 0;
+  if (g_tune_split && pl.unit_groups == 1 && g_tune_force_ctas == 0) {
+    const int k = ctas / pl.tiles;
+    if (k >= 2 && k <= pl.G && pl.tiles * k * 10 >= ctas * 9) {
+      pl.split = k;
+      pl.ctas = pl.tiles * k;
+    }
+  }
   return pl;
 }
 
@@ -680,6 +706,7 @@ int er_gemm_tuning(int key, int value) {
   if (key == 1 && value >= 0) { g_tune_force_ctas = value; return ER_OK; }
   if (key == 2 && value >= 0) { g_tune_dbg = value; return ER_OK; }
   if (key == 3 && (value == 0 || value == 1)) { g_tune_pdl = value; return ER_OK; }
+  if (key == 4 && (value == 0 || value == 1)) { g_tune_split = value; return ER_OK; }
   return ER_ERR_SHAPE;
 }
 
@@ -728,6 +755,8 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
   gp.M = (int)M; gp.N = (int)N; gp.K = (int)K;
   gp.G = pl.G; gp.ntiles = pl.ntiles; gp.tiles = pl.tiles; gp.unit_groups = pl.unit_groups; gp.units = (int)pl.units;
   gp.uq = (int)(pl.units / pl.ctas); gp.ur = (int)(pl.units % pl.ctas);
+  gp.split = pl.split;
+  if (pl.split > 0) { gp.uq = pl.G; gp.ur = 0; }
   gp.dbg = g_tune_dbg;
 #ifdef ER_GEMM_TRACE
   gp.trace = g_trace;
