@@ -232,6 +232,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   const int ge = range_begin(p.uq, p.ur, p.split, cta + 1) * ug;
   const int n_it = (int)(ge - gb);
 #ifdef ER_GEMM_TRACE
+  if (p.trace && threadIdx.x == 0) { unsigned long long gt; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(gt)); p.trace[1024 + blockIdx.x * 2] = gt; }
   unsigned tr_sum[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   unsigned tr_sum2[8] = {0, 0, 0, 0, 0, 0, 0, 0};
   unsigned tr_prev = (unsigned)clock();
@@ -259,6 +260,9 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   // The next kernel may be scheduled as soon as SMs free up (it waits at its own griddepcontrol.wait).
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+#ifdef ER_GEMM_TRACE
+  if (p.trace && threadIdx.x == 0) { unsigned long long gt; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(gt)); p.trace[2048 + blockIdx.x * 4] = gt; }
+#endif
   ER_TR(0);
 
   if (warp == 0) {
@@ -519,6 +523,9 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
     // what the barrier made visible to the leader); last arriver: acq_rel ticket -> bar.sync -> ld.cg of the others'
     // partials.  No per-thread __threadfence on either side.
     ER_TR2(0);
+#ifdef ER_GEMM_TRACE
+    if (p.trace && leader) { unsigned long long gt; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(gt)); p.trace[2048 + blockIdx.x * 4 + 1] = gt; }
+#endif
     if (set == 0 && (pend_tile[0] >= 0 || pend_tile[1] >= 0)) {
       named_bar_sync(7, kSetThreads);
       ER_TR2(1);
@@ -546,6 +553,9 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
       }
       named_bar_sync(7, kSetThreads);
       ER_TR2(2);
+#ifdef ER_GEMM_TRACE
+      if (p.trace && leader) { unsigned long long gt; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(gt)); p.trace[2048 + blockIdx.x * 4 + 2] = gt; p.trace[2048 + blockIdx.x * 4 + 3] = last_flag[0] | (last_flag[1] << 1); }
+#endif
       constexpr int kChunk = CW <= 8 ? 6 : (CW <= 16 ? 3 : 1);   // contributors whose loads are in flight together
 #pragma unroll
       for (int k = 0; k < 2; ++k) {
@@ -585,6 +595,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   tc_fence_after();
   if (warp == 1) tmem_dealloc<kTmemCols>(tmem);
 #ifdef ER_GEMM_TRACE
+  if (p.trace && threadIdx.x == 0) { unsigned long long gt; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(gt)); p.trace[1024 + blockIdx.x * 2 + 1] = gt; }
   if (p.trace && blockIdx.x == p.dbg_cta && lane == 0)
     for (int i = 0; i < 8; ++i) { p.trace[warp * 8 + i] = tr_sum[i]; p.trace[256 + warp * 8 + i] = tr_sum2[i]; }
 #endif
