@@ -450,7 +450,7 @@ def product_arm(args):
             "clocks": sampler.summary(),
             "e2e": e2e,
             "gpu_launches": launches_per_step * args.steps,
-            "roofline": {"bound": "hbm", "kernel": "w4a16_gemm_kernel<16> (all M<=16 launches of the step)",
+            "roofline": {"bound": "hbm", "kernel": "w4a16_gemm_kernel<16, *> (all M<=16 launches of the step; QKV, O, down run the cluster variant)",
                          "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
                          "frac": round(achieved / peak, 4), "traffic": NCU_TRAFFIC_BYTES, "peak_source": peak_src,
                          "bytes_per_launch": round(k16_bytes / k16_n), "us_per_launch": round(k16_ms / k16_n * 1e3, 2)},

@@ -103,7 +103,7 @@ int er_quantize_pack(const void* w_bf16, int64_t N, int64_t K, int64_t ldw_elems
  * tensor cores with fp32 accumulation per 128-k group; the same accumulator receives -136 * sum_k x[m][k]
  * (the offset, through a constant operand tile), so it holds sum_k x * q up to fp32 rounding; each group's
  * sum is multiplied by its fp32 scale and added in fp32 (no rounding of q*s); split-K partials are reduced
- * in ascending CTA order (deterministic).
+ * in ascending CTA order, or inside a thread-block cluster in rank order (both deterministic).
  * Launch: one persistent kernel, launched with programmatic stream serialization; it touches no global
  * memory before griddepcontrol.wait, so ordering against earlier work in the stream is the usual one. */
 int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems,

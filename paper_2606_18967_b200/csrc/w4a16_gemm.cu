@@ -77,6 +77,7 @@ struct GemmParams {
   int units;           // tiles * G / unit_groups (< 2^31, checked on the host)
   int uq, ur;          // units / CTAs and units % CTAs: CTA c owns units [c*uq + min(c, ur), ...)
   int split;           // > 0: tile split (see range_begin); uq = groups per tile
+  int cluster;         // > 1: the `split` CTAs of a tile form one thread-block cluster and reduce through DSMEM
   int y_f32;
   int64_t ldy;
   void* y;
@@ -207,7 +208,7 @@ __device__ __forceinline__ int owner_of(int uq, int ur, int split, int u) {
 
 __device__ __forceinline__ void named_bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
-template <int MPAD>
+template <int MPAD, bool kClusterMode>
 __global__ void __launch_bounds__(kThreads, 1)
 w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
   using C = Cfg<MPAD>;
@@ -231,6 +232,9 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   const int gb = range_begin(p.uq, p.ur, p.split, cta) * ug;        // first global group index of this CTA
   const int ge = range_begin(p.uq, p.ur, p.split, cta + 1) * ug;
   const int n_it = (int)(ge - gb);
+  static_assert(!kClusterMode || MPAD == 16, "the host only uses clusters at M <= 16");
+  float cl_acc[kClusterMode ? C::kCW : 1];      // cluster mode: set 0's sum over this CTA's part of its tile ...
+  int cl_tile = -1;                     // ... and the tile
 #ifdef ER_GEMM_TRACE
   if (p.trace && threadIdx.x == 0) { unsigned long long gt; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(gt)); p.trace[1024 + blockIdx.x * 2] = gt; }
   unsigned tr_sum[8] = {0, 0, 0, 0, 0, 0, 0, 0};
@@ -503,6 +507,13 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
         //      finished after the main loop (the reduction's round trips would otherwise stall the pipeline) ----
         if (seg_len == p.G) {
           store_tile(tile, acc);
+        } else if (kClusterMode && p.cluster > 1) {   // reduced over the cluster at the end of the kernel (one segment
+                                                      // per CTA)
+          if constexpr (kClusterMode) {
+#pragma unroll
+            for (int m = 0; m < CW; ++m) cl_acc[m] = acc[m];
+          }
+          cl_tile = tile;
         } else {
           const int k = (it == 0 ? 0 : 1);
           const int m0 = (tile / p.ntiles) * MPAD + half * CW;
@@ -594,6 +605,48 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   __syncthreads();
   tc_fence_after();
   if (warp == 1) tmem_dealloc<kTmemCols>(tmem);
+
+  // ---- cluster mode: the k CTAs of a tile add their sums through distributed shared memory (an L2 ticket plus
+  //      partial loads costs two ~1 us round trips; here it is two cluster barriers and remote shared-memory stores).
+  //      Rank r > 0 writes its [MPAD x 128] fp32 tile into slot r - 1 of rank 0's (now idle) stage memory; rank 0
+  //      adds the slots in rank order and stores the tile.  Deterministic. ----
+  if constexpr (kClusterMode) if (p.cluster > 1) {
+    uint32_t rank;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
+    // #1: every CTA of the cluster is past its main loop: rank 0's stage memory is idle
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    const bool set0 = (warp >= kSetWarp0 && warp < kSetWarp0 + 8);
+    const int row = (warp & 3) * 32 + lane, hf = ((warp - kSetWarp0) >> 2) & 1;
+    if (set0 && rank != 0 && cl_tile >= 0) {
+      uint32_t remote;
+      asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(smem)), "r"(0));
+      remote += (((rank - 1) * MPAD + hf * C::kCW) * kTileN + row) * 4;
+#pragma unroll
+      for (int m = 0; m < C::kCW; ++m)
+        asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(remote + m * kTileN * 4), "f"(cl_acc[m]) : "memory");
+    }
+    // #2: the remote stores are visible to rank 0
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    if (set0 && rank == 0 && cl_tile >= 0) {
+      const float* slots = reinterpret_cast<const float*>(smem);
+      for (int r = 1; r < p.cluster; ++r)
+#pragma unroll
+        for (int m = 0; m < C::kCW; ++m) cl_acc[m] += slots[((r - 1) * MPAD + hf * C::kCW + m) * kTileN + row];
+      const int n = (cl_tile % p.ntiles) * kTileN + row, m0 = (cl_tile / p.ntiles) * MPAD + hf * C::kCW;
+      const int mvalid = min(C::kCW, p.M - m0);
+      if (p.y_f32) {
+        float* y = reinterpret_cast<float*>(p.y);
+#pragma unroll
+        for (int m = 0; m < C::kCW; ++m)
+          if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = cl_acc[m];
+      } else {
+        __nv_bfloat16* y = reinterpret_cast<__nv_bfloat16*>(p.y);
+#pragma unroll
+        for (int m = 0; m < C::kCW; ++m)
+          if (m < mvalid) y[(size_t)(m0 + m) * p.ldy + n] = __float2bfloat16_rn(cl_acc[m]);
+      }
+    }
+  }
 #ifdef ER_GEMM_TRACE
   if (p.trace && threadIdx.x == 0) { unsigned long long gt; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(gt)); p.trace[1024 + blockIdx.x * 2 + 1] = gt; }
   if (p.trace && blockIdx.x == p.dbg_cta && lane == 0)
@@ -648,9 +701,12 @@ int g_tune_split = 1;        // tile split where it applies (key 4)
 int g_tune_force_ctas = 0;  // > 0: use this many CTAs (tests / sweeps); 0 = one per SM
 
 struct Plan {
-  int mpad, mchunks, ntiles, tiles, G, unit_groups, ctas, split;
+  int mpad, mchunks, ntiles, tiles, G, unit_groups, ctas, split, cluster;
   long long units;
 };
+
+int g_tune_cluster = 1;      // cluster mode where it applies (key 5)
+int max_active_clusters16(int c);
 
 int mpad_of(int64_t M) { return M <= 16 ? 16 : (M <= 32 ? 32 : 64); }
 
@@ -677,6 +733,19 @@ Plan make_plan(int64_t M, int64_t N, int64_t K) {
       pl.ctas = pl.tiles * k;
     }
   }
+  // cluster mode (M <= 16): the parts of a tile are one thread-block cluster and reduce through distributed shared
+  // memory.  The cluster size is limited by how many clusters of one-CTA-per-SM footprint the GPCs can hold at once.
+  pl.cluster = 1;
+  if (g_tune_cluster && pl.mpad == 16 && pl.unit_groups == 1 && g_tune_force_ctas == 0 && pl.mchunks == 1) {
+    for (int c = 4; c >= 2; --c) {
+      if (c <= pl.G && max_active_clusters16(c) >= pl.tiles && pl.tiles * c * 10 >= ctas * 7) {
+        pl.cluster = c;
+        pl.split = c;
+        pl.ctas = pl.tiles * c;
+        break;
+      }
+    }
+  }
   return pl;
 }
 
@@ -684,11 +753,11 @@ size_t workspace_for(int mpad) {
   return ER_GEMM_COUNTER_BYTES + (size_t)er::sm_count() * 2 * mpad * kTileN * sizeof(float);
 }
 
-template <int MPAD>
+template <int MPAD, bool kCl>
 int launch(const CUtensorMap& mx, const GemmParams& gp, const Plan& pl, cudaStream_t stream) {
   static bool attr_set = false;
   if (!attr_set) {
-    ER_CUDA_TRY(cudaFuncSetAttribute(w4a16_gemm_kernel<MPAD>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    ER_CUDA_TRY(cudaFuncSetAttribute(w4a16_gemm_kernel<MPAD, kCl>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      Cfg<MPAD>::kSmem));
     attr_set = true;
   }
@@ -697,13 +766,46 @@ int launch(const CUtensorMap& mx, const GemmParams& gp, const Plan& pl, cudaStre
   cfg.blockDim = dim3(kThreads);
   cfg.dynamicSmemBytes = Cfg<MPAD>::kSmem;
   cfg.stream = stream;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   attr[0].val.programmaticStreamSerializationAllowed = g_tune_pdl;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  ER_CUDA_TRY(cudaLaunchKernelEx(&cfg, w4a16_gemm_kernel<MPAD>, mx, gp));
+  if (pl.cluster > 1) {
+    attr[1].id = cudaLaunchAttributeClusterDimension;
+    attr[1].val.clusterDim.x = (unsigned)pl.cluster;
+    attr[1].val.clusterDim.y = 1;
+    attr[1].val.clusterDim.z = 1;
+    cfg.numAttrs = 2;
+  }
+  ER_CUDA_TRY(cudaLaunchKernelEx(&cfg, w4a16_gemm_kernel<MPAD, kCl>, mx, gp));
   return ER_OK;
+}
+
+// how many clusters of c CTAs of the M <= 16 kernel (one CTA per SM) can be resident at once; cached
+int max_active_clusters16(int c) {
+  static int cache[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
+  if (c < 2 || c > 8) return 0;
+  if (cache[c] != 0) return cache[c] < 0 ? 0 : cache[c];
+  cudaFuncSetAttribute(w4a16_gemm_kernel<16, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg<16>::kSmem);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(c * 64));
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = Cfg<16>::kSmem;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)c;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  int n = 0;
+  if (cudaOccupancyMaxActiveClusters(&n, w4a16_gemm_kernel<16, true>, &cfg) != cudaSuccess) {
+    (void)cudaGetLastError();
+    n = 0;
+  }
+  cache[c] = n > 0 ? n : -1;
+  return n;
 }
 
 }  // namespace
@@ -718,6 +820,7 @@ int er_gemm_tuning(int key, int value) {
   if (key == 2 && value >= 0) { g_tune_dbg = value; return ER_OK; }
   if (key == 3 && (value == 0 || value == 1)) { g_tune_pdl = value; return ER_OK; }
   if (key == 4 && (value == 0 || value == 1)) { g_tune_split = value; return ER_OK; }
+  if (key == 5 && (value == 0 || value == 1)) { g_tune_cluster = value; return ER_OK; }
   return ER_ERR_SHAPE;
 }
 
@@ -767,6 +870,7 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
   gp.G = pl.G; gp.ntiles = pl.ntiles; gp.tiles = pl.tiles; gp.unit_groups = pl.unit_groups; gp.units = (int)pl.units;
   gp.uq = (int)(pl.units / pl.ctas); gp.ur = (int)(pl.units % pl.ctas);
   gp.split = pl.split;
+  gp.cluster = pl.cluster;
   if (pl.split > 0) { gp.uq = pl.G; gp.ur = 0; }
   gp.dbg = g_tune_dbg;
 #ifdef ER_GEMM_TRACE
@@ -779,9 +883,9 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
   gp.counters = reinterpret_cast<int*>(workspace);
   gp.partials = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + ER_GEMM_COUNTER_BYTES);
   cudaStream_t s = (cudaStream_t)stream;
-  if (pl.mpad == 16) return launch<16>(mx, gp, pl, s);
-  if (pl.mpad == 32) return launch<32>(mx, gp, pl, s);
-  return launch<64>(mx, gp, pl, s);
+  if (pl.mpad == 16) return pl.cluster > 1 ? launch<16, true>(mx, gp, pl, s) : launch<16, false>(mx, gp, pl, s);
+  if (pl.mpad == 32) return launch<32, false>(mx, gp, pl, s);
+  return launch<64, false>(mx, gp, pl, s);
 }
 
 }  // extern "C"

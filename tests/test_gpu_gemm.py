@@ -239,3 +239,24 @@ def test_programmatic_dependent_launch_does_not_change_results():
         outs.append(y.clone())
     lib.er_gemm_tuning(3, 1)
     assert torch.equal(outs[0], outs[1])
+
+
+@pytest.mark.parametrize("mode", ["cluster", "tile_split", "stream_k"])
+def test_partition_modes_agree_with_the_oracle_and_are_deterministic(mode):
+    # the same problem under the three work partitions (cluster reduction through DSMEM; k parts per tile with
+    # an L2 ticket; stream-K ranges): each within tolerance of the oracle and bit-identical run to run
+    N, K, M = 4608, 3584, 16
+    w = I.weight_bf16(N, K, I.seed_of("modes", "w"), device=DEV)
+    x = I.activation_bf16(M, K, I.seed_of("modes", "x"), device=DEV)
+    qw, sc = er.quantize_pack(w)
+    lib = er.load()
+    lib.er_gemm_tuning(5, 1 if mode == "cluster" else 0)
+    lib.er_gemm_tuning(4, 0 if mode == "stream_k" else 1)
+    try:
+        y1 = _sampled_columns_check(x, qw, sc, N, K, 7, mode)
+        y2 = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
+        torch.cuda.synchronize()
+        assert torch.equal(y1, y2)
+    finally:
+        lib.er_gemm_tuning(5, 1)
+        lib.er_gemm_tuning(4, 1)
