@@ -91,6 +91,18 @@ int er_gemm_workspace_init(void* workspace, size_t workspace_bytes, void* stream
 int er_quantize_pack(const void* w_bf16, int64_t N, int64_t K, int64_t ldw_elems, int group,
                      void* qweight_out, void* scales_out, void* stream);
 
+/* The same for `count` weight matrices in as few launches as possible (the refresh of a decoder layer or of the
+ * whole model: every FFN / QKVO weight, every RL step).  `descs` is a HOST array; the pointers
+ * inside are DEVICE pointers with the meaning and constraints of er_quantize_pack.  Everything is validated
+ * before anything is launched.  Results are identical to `count` separate calls. */
+typedef struct {
+  const void* w;   /* bf16 [N][K], row stride ldw elements */
+  int64_t N, K, ldw;
+  void* qweight;   /* out: ER_PACK_V2 */
+  void* scales;    /* out: bf16 [K/128][N] */
+} er_linear_desc;
+int er_quantize_pack_batched(const er_linear_desc* descs, int count, int group, void* stream);
+
 /* (1) Drafter linear:  Y[m][n] = sum_k X[m][k] * q[n][k] * s[k/128][n].
  *   x_bf16   [M][K] bf16, row stride ldx_elems; base 16-byte aligned, ldx_elems % 8 == 0; M >= 1
  *   qweight, scales  as produced by er_quantize_pack (any nibble incl. -8 is legal); N % 128 == 0,

@@ -90,14 +90,14 @@ __device__ __noinline__ uint2 pack16_div(const uint16_t* src, float s) {
   return make_uint2(pack8<true>(r0, s, 0.f), pack8<true>(r1, s, 0.f));
 }
 
-__global__ void __launch_bounds__(kThreads) quantize_pack_kernel(const uint16_t* __restrict__ w, int64_t N,
-                                                                 int64_t K, int64_t ldw,
-                                                                 uint32_t* __restrict__ qweight,
-                                                                 uint16_t* __restrict__ scales, int vec256) {
+// One CTA quantizes the tile (bx: 512-k tile, by: 32-row tile) of one weight matrix.
+__device__ __forceinline__ void quantize_tile(const uint16_t* __restrict__ w, int64_t N, int64_t K, int64_t ldw,
+                                              uint32_t* __restrict__ qweight, uint16_t* __restrict__ scales,
+                                              int vec256, unsigned bx, unsigned by) {
   __shared__ uint16_t s_scales[kTileK / ER_GROUP][kTileRows];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t n0 = (int64_t)blockIdx.y * kTileRows;
-  const int64_t k = (int64_t)blockIdx.x * kTileK + lane * 16;
+  const int64_t n0 = (int64_t)by * kTileRows;
+  const int64_t k = (int64_t)bx * kTileK + lane * 16;
 
   U8 v[kIters];
   bool ok[kIters];
@@ -152,9 +152,39 @@ __global__ void __launch_bounds__(kThreads) quantize_pack_kernel(const uint16_t*
   __syncthreads();
   if (threadIdx.x < (kTileK / ER_GROUP) * kTileRows) {
     const int g = threadIdx.x >> 5, r = threadIdx.x & 31;
-    const int64_t gg = ((int64_t)blockIdx.x * kTileK >> 7) + g, n = n0 + r;
+    const int64_t gg = ((int64_t)bx * kTileK >> 7) + g, n = n0 + r;
     if (n < N && gg < (K >> 7)) scales[gg * N + n] = s_scales[g][r];
   }
+}
+
+__global__ void __launch_bounds__(kThreads) quantize_pack_kernel(const uint16_t* __restrict__ w, int64_t N,
+                                                                 int64_t K, int64_t ldw,
+                                                                 uint32_t* __restrict__ qweight,
+                                                                 uint16_t* __restrict__ scales, int vec256) {
+  quantize_tile(w, N, K, ldw, qweight, scales, vec256, blockIdx.x, blockIdx.y);
+}
+
+// Several weight matrices in one launch (the refresh of a whole decoder layer / model): a 1-D grid over the tiles of
+// all of them, so that the tails of the small matrices overlap with the large ones instead of each paying its own
+// launch and drain.
+constexpr int kMaxBatch = 8;
+struct BatchParams {
+  const uint16_t* w[kMaxBatch];
+  uint32_t* qweight[kMaxBatch];
+  uint16_t* scales[kMaxBatch];
+  int64_t N[kMaxBatch], K[kMaxBatch], ldw[kMaxBatch];
+  unsigned kt[kMaxBatch];          // 512-k tiles per row tile
+  unsigned first[kMaxBatch + 1];   // first CTA of every matrix
+  int vec256[kMaxBatch];
+  int count;
+};
+__global__ void __launch_bounds__(kThreads) quantize_pack_batched_kernel(const __grid_constant__ BatchParams bp) {
+  int t = 0;
+  while (t + 1 < bp.count && blockIdx.x >= bp.first[t + 1]) ++t;
+  const unsigned local = blockIdx.x - bp.first[t];
+  // k tiles fastest, as in the single-matrix grid: consecutive CTAs stream consecutive bytes of the same rows
+  quantize_tile(bp.w[t], bp.N[t], bp.K[t], bp.ldw[t], bp.qweight[t], bp.scales[t], bp.vec256[t], local % bp.kt[t],
+                local / bp.kt[t]);
 }
 
 __global__ void unpack_codes_kernel(const uint32_t* __restrict__ qweight, int64_t words, int64_t K,
@@ -197,6 +227,45 @@ int er_quantize_pack(const void* w_bf16, int64_t N, int64_t K, int64_t ldw_elems
       reinterpret_cast<const uint16_t*>(w_bf16), N, K, ldw_elems, reinterpret_cast<uint32_t*>(qweight_out),
       reinterpret_cast<uint16_t*>(scales_out), vec256);
   ER_CUDA_TRY(cudaGetLastError());
+  return ER_OK;
+}
+
+int er_quantize_pack_batched(const er_linear_desc* descs, int count, int group, void* stream) {
+  if (count < 0) return ER_ERR_SHAPE;
+  if (count == 0) return ER_OK;
+  if (!descs) return ER_ERR_NULL;
+  for (int i = 0; i < count; ++i) {           // validate everything before anything is launched
+    const er_linear_desc& d = descs[i];
+    if (!d.w || !d.qweight || !d.scales) return ER_ERR_NULL;
+    if (group != ER_GROUP || d.N < 128 || d.N % 128 != 0 || d.K < ER_GROUP || d.K % ER_GROUP != 0 || d.ldw < d.K)
+      return ER_ERR_SHAPE;
+    if ((d.N + kTileRows - 1) / kTileRows > 65535) return ER_ERR_SHAPE;
+    if (!er::aligned16(d.w) || !er::aligned16(d.qweight) || (d.ldw % 8) != 0 ||
+        (reinterpret_cast<uintptr_t>(d.scales) & 1u))
+      return ER_ERR_ALIGN;
+  }
+  int st = er::check_arch();
+  if (st != ER_OK) return st;
+  for (int base = 0; base < count; base += kMaxBatch) {
+    BatchParams bp;
+    bp.count = count - base < kMaxBatch ? count - base : kMaxBatch;
+    unsigned long long total = 0;
+    for (int i = 0; i < bp.count; ++i) {
+      const er_linear_desc& d = descs[base + i];
+      bp.w[i] = reinterpret_cast<const uint16_t*>(d.w);
+      bp.qweight[i] = reinterpret_cast<uint32_t*>(d.qweight);
+      bp.scales[i] = reinterpret_cast<uint16_t*>(d.scales);
+      bp.N[i] = d.N; bp.K[i] = d.K; bp.ldw[i] = d.ldw;
+      bp.kt[i] = (unsigned)((d.K + kTileK - 1) / kTileK);
+      bp.vec256[i] = ((reinterpret_cast<uintptr_t>(d.w) & 31u) == 0 && (d.ldw % 16) == 0) ? 1 : 0;
+      bp.first[i] = (unsigned)total;
+      total += (unsigned long long)bp.kt[i] * (unsigned long long)((d.N + kTileRows - 1) / kTileRows);
+      if (total > 0x7FFFFFFFull) return ER_ERR_SHAPE;
+    }
+    for (int i = bp.count; i <= kMaxBatch; ++i) bp.first[i] = (unsigned)total;
+    quantize_pack_batched_kernel<<<(unsigned)total, kThreads, 0, (cudaStream_t)stream>>>(bp);
+    ER_CUDA_TRY(cudaGetLastError());
+  }
   return ER_OK;
 }
 

@@ -20,6 +20,12 @@ COUNTER_BYTES = 16384
 _lib = None
 
 
+class LinearDesc(ctypes.Structure):
+    """er_linear_desc of include/er.h."""
+    _fields_ = [("w", ctypes.c_void_p), ("N", ctypes.c_int64), ("K", ctypes.c_int64), ("ldw", ctypes.c_int64),
+                ("qweight", ctypes.c_void_p), ("scales", ctypes.c_void_p)]
+
+
 class ErError(RuntimeError):
     def __init__(self, status: int, where: str):
         lib = load()
@@ -53,6 +59,8 @@ def load() -> ctypes.CDLL:
     lib.er_gemm_workspace_init.argtypes = [vp, sz, vp]
     lib.er_quantize_pack.restype = ctypes.c_int
     lib.er_quantize_pack.argtypes = [vp, i64, i64, i64, ctypes.c_int, vp, vp, vp]
+    lib.er_quantize_pack_batched.restype = ctypes.c_int
+    lib.er_quantize_pack_batched.argtypes = [ctypes.POINTER(LinearDesc), ctypes.c_int, ctypes.c_int, vp]
     lib.er_w4a16_gemm.restype = ctypes.c_int
     lib.er_w4a16_gemm.argtypes = [vp, i64, i64, i64, vp, vp, i64, ctypes.c_int, vp, i64, ctypes.c_int, vp, sz, vp]
     lib.er_w4a16_gemm_simt.restype = ctypes.c_int
@@ -131,6 +139,20 @@ def quantize_pack(w: torch.Tensor, qweight: torch.Tensor | None = None, scales: 
     _check(load().er_quantize_pack(w.data_ptr(), N, K, w.stride(0), group, qweight.data_ptr(), scales.data_ptr(),
                                    _stream(w)), "er_quantize_pack")
     return qweight, scales
+
+
+def quantize_pack_batched(items, group: int = GROUP):
+    """items: iterable of (w, qweight, scales) device tensors; one call for all of them (er_quantize_pack_batched)."""
+    items = list(items)
+    if not items:
+        return
+    arr = (LinearDesc * len(items))()
+    for d, (w, qweight, scales) in zip(arr, items):
+        _cuda(w, "w")
+        assert w.dtype == torch.bfloat16 and w.dim() == 2 and w.stride(1) == 1
+        d.w, d.N, d.K, d.ldw = w.data_ptr(), w.shape[0], w.shape[1], w.stride(0)
+        d.qweight, d.scales = qweight.data_ptr(), scales.data_ptr()
+    _check(load().er_quantize_pack_batched(arr, len(items), group, _stream(items[0][0])), "er_quantize_pack_batched")
 
 
 def w4a16_gemm(x: torch.Tensor, qweight: torch.Tensor, scales: torch.Tensor, out_dtype=torch.bfloat16,

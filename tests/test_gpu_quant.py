@@ -89,3 +89,22 @@ def test_sampled_groups_of_a_7b_layer():
         G = K // 128
         got = qw.cpu().numpy().view(np.uint32).reshape(-1)[T * G * 2048:(T + 1) * G * 2048]
         assert np.array_equal(got, qr.reshape(-1))
+
+
+def test_batched_equals_separate_calls():
+    # er_quantize_pack_batched: several matrices (different shapes, one strided) in one launch, bit-identical to
+    # separate calls; more matrices than fit one launch (> 8) are chained
+    shapes = [(128, 128), (256, 1152), (384, 640), (128, 4096), (512, 512), (128, 256), (256, 128), (128, 1024),
+              (640, 384), (128, 128)]
+    items, refs = [], []
+    for i, (N, K) in enumerate(shapes):
+        w = I.weight_bf16(N, K + (16 if i == 2 else 0), I.seed_of("batched", i), device=DEV)[:, :K]
+        q1, s1 = er.quantize_pack(w)
+        q2 = torch.zeros_like(q1)
+        s2 = torch.zeros_like(s1)
+        items.append((w, q2, s2))
+        refs.append((q1, s1))
+    er.quantize_pack_batched(items)
+    torch.cuda.synchronize()
+    for (w, q2, s2), (q1, s1) in zip(items, refs):
+        assert torch.equal(q1, q2) and torch.equal(s1.view(torch.int16), s2.view(torch.int16))
