@@ -260,3 +260,17 @@ def test_partition_modes_agree_with_the_oracle_and_are_deterministic(mode):
     finally:
         lib.er_gemm_tuning(5, 1)
         lib.er_gemm_tuning(4, 1)
+
+
+@pytest.mark.parametrize("M", [1, 16, 64])
+def test_heavy_tailed_activations_stay_within_tolerance(M):
+    # the -136 offset of the stored nibble is folded into the contraction (fp32 accumulation of x * (136 + q) and of
+    # -136 * x): activations with 100x outliers (as LLM hidden states have) must not cost accuracy
+    N, K = 512, 3584
+    w = I.weight_bf16(N, K, I.seed_of("tail", "w"), device=DEV)
+    qw, sc = er.quantize_pack(w)
+    g = torch.Generator(device="cpu").manual_seed(I.seed_of("tail", "x", M) % (2 ** 31))
+    x = torch.randn(M, K, generator=g)
+    mask = torch.rand(M, K, generator=g) < 0.002
+    x = torch.where(mask, x * 100.0, x).to(torch.bfloat16).to(DEV)
+    _check(x, qw, sc)
