@@ -58,7 +58,7 @@ struct Cfg {
   static constexpr int kSmem = kStages * kStageBytes + kFixed;
   static constexpr uint32_t kTxBytes = kWBytes + kXBytes + kScaleBytes;
   static constexpr int kCW = MPAD / 2;                     // accumulator columns per thread (half of the batch rows)
-  static constexpr bool kSubInWorkers = (MPAD > 32);      // see dequant_word
+  static constexpr bool kSubInWorkers = (MPAD > 16);      // see dequant_word
   static constexpr bool kEpiFirst = (MPAD > 32);           // register pressure: read back before converting
   // TMEM: every set owns kBuf (A operand, accumulator) pairs.  Two pairs (M <= 16, where the columns allow it)
   // let a set convert group i + 1 while the MMAs of group i are still in flight.
@@ -150,7 +150,8 @@ __device__ __forceinline__ uint32_t lop3_and_or(uint32_t a, uint32_t mask, uint3
 // contraction: eight more MMAs per group with a constant A tile of -136 add -136 * sum_k x to the accumulator.
 // (An fp16 A operand would need 5 logic ops, but tcgen05.mma.kind::f16 faults on fp16 A x bf16 B.)
 // kSub: remove the 136 here with one packed fma per pair (used where the tensor pipe, not the logic pipe, is the
-// busier one: at N = 64 the eight constant-tile MMAs per group cost more than the subtracts).
+// busier one: at N >= 32 the eight constant-tile MMAs per group cost more than the subtracts, which issue on the
+// FMA pipe beside the logic-pipe shifts and lop3s).
 template <bool kSub>
 __device__ __forceinline__ void dequant_word(uint32_t w, uint32_t* a) {
 #pragma unroll
