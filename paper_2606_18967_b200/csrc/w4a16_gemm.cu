@@ -52,7 +52,11 @@ struct Cfg {
   static constexpr int kXBytes = MPAD * 128 * 2;           // two boxes of [MPAD x 64] bf16
   static constexpr int kStageBytes = ((kWBytes + kXBytes + kScaleBytes + 1023) / 1024) * 1024;
   static constexpr int kRedBytes = (kSets - 1) * MPAD * kTileN * 4;   // partial sums of sets 1.. handed to set 0
-  static constexpr int kFixed = kRedBytes + 1024 /*align slack*/ + 512 /*barriers*/;
+  // cluster mode (M <= 16): up to 3 [MPAD x 128] fp32 slots that the other CTAs of the cluster write into rank 0;
+  // a region of their own, so the writers need not wait for rank 0's pipeline to drain (the ring depth is not
+  // critical: 8 and 16 stages measure the same)
+  static constexpr int kSlotBytes = (MPAD == 16) ? 3 * MPAD * kTileN * 4 : 0;
+  static constexpr int kFixed = kRedBytes + kSlotBytes + 1024 /*align slack*/ + 512 /*barriers*/;
   static constexpr int kStagesRaw = (kSmemLimit - kFixed) / kStageBytes;
   static constexpr int kStages = kStagesRaw > kMaxStages ? kMaxStages : kStagesRaw;
   static constexpr int kSmem = kStages * kStageBytes + kFixed;
@@ -218,7 +222,8 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   extern __shared__ uint8_t smem_raw[];
   uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   float* red = reinterpret_cast<float*>(smem + S * C::kStageBytes);             // [kSets-1][MPAD][128]
-  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + S * C::kStageBytes + C::kRedBytes);
+  uint8_t* slots_base = smem + S * C::kStageBytes + C::kRedBytes;               // cluster slots (see Cfg)
+  uint64_t* bars = reinterpret_cast<uint64_t*>(smem + S * C::kStageBytes + C::kRedBytes + C::kSlotBytes);
   uint64_t* full = bars;                        // [S]     TMA landed
   uint64_t* empty = bars + kMaxStages;          // [S]     the group's MMAs completed: the stage may be refilled
   uint64_t* a_full = bars + 2 * kMaxStages;     // [kSets][kBuf] the A operand is written, its accumulator drained
@@ -260,6 +265,9 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);
+  if constexpr (kClusterMode) {   // "I have started": waited for before the first remote shared-memory access
+    if (p.cluster > 1) asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
+  }
   // Programmatic dependent launch: everything above touched no global memory, so it may overlap the tail of the
   // previous kernel in the stream; from here on its results (X, the packed weights, the workspace) are needed.
   // The next kernel may be scheduled as soon as SMs free up (it waits at its own griddepcontrol.wait).
@@ -608,28 +616,28 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   if (warp == 1) tmem_dealloc<kTmemCols>(tmem);
 
   // ---- cluster mode: the k CTAs of a tile add their sums through distributed shared memory (an L2 ticket plus
-  //      partial loads costs two ~1 us round trips; here it is two cluster barriers and remote shared-memory stores).
-  //      Rank r > 0 writes its [MPAD x 128] fp32 tile into slot r - 1 of rank 0's (now idle) stage memory; rank 0
+  //      partial loads costs two ~1 us round trips; here it is remote shared-memory stores and one cluster barrier).
+  //      Rank r > 0 writes its [MPAD x 128] fp32 tile into slot r - 1 of rank 0's slot region; rank 0
   //      adds the slots in rank order and stores the tile.  Deterministic. ----
   if constexpr (kClusterMode) if (p.cluster > 1) {
     uint32_t rank;
     asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(rank));
-    // #1: every CTA of the cluster is past its main loop: rank 0's stage memory is idle
-    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.aligned;" ::: "memory");   // every CTA of the cluster has started (long ago)
     const bool set0 = (warp >= kSetWarp0 && warp < kSetWarp0 + 8);
     const int row = (warp & 3) * 32 + lane, hf = ((warp - kSetWarp0) >> 2) & 1;
     if (set0 && rank != 0 && cl_tile >= 0) {
       uint32_t remote;
-      asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(smem)), "r"(0));
+      asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(remote) : "r"(smem_u32(slots_base)), "r"(0));
       remote += (((rank - 1) * MPAD + hf * C::kCW) * kTileN + row) * 4;
 #pragma unroll
       for (int m = 0; m < C::kCW; ++m)
         asm volatile("st.shared::cluster.f32 [%0], %1;" ::"r"(remote + m * kTileN * 4), "f"(cl_acc[m]) : "memory");
     }
-    // #2: the remote stores are visible to rank 0
+    // one cluster barrier: the remote stores are visible to rank 0 (rank 0's slot region is never touched by its own
+    // pipeline, so the writers did not have to wait for it)
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
     if (set0 && rank == 0 && cl_tile >= 0) {
-      const float* slots = reinterpret_cast<const float*>(smem);
+      const float* slots = reinterpret_cast<const float*>(slots_base);
       for (int r = 1; r < p.cluster; ++r)
 #pragma unroll
         for (int m = 0; m < C::kCW; ++m) cl_acc[m] += slots[((r - 1) * MPAD + hf * C::kCW + m) * kTileN + row];
