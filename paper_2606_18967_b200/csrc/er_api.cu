@@ -13,13 +13,26 @@ int check_arch() {
   return major == 10 ? ER_OK : ER_ERR_ARCH;
 }
 
+int current_device() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) {
+    (void)cudaGetLastError();
+    return 0;
+  }
+  return dev;
+}
+
+// Per-device cache (a racing first call from two host threads writes the same value twice).
 int sm_count() {
-  static int cached = 0;
-  if (cached) return cached;
-  int dev = 0, n = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) return 148;
-  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) return 148;
-  cached = n;
+  static int cached[kMaxDevices] = {};
+  const int dev = current_device();
+  if (dev >= 0 && dev < kMaxDevices && cached[dev]) return cached[dev];
+  int n = 0;
+  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+    (void)cudaGetLastError();
+    return 148;
+  }
+  if (dev >= 0 && dev < kMaxDevices) cached[dev] = n;
   return n;
 }
 }  // namespace er

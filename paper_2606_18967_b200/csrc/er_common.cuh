@@ -13,6 +13,10 @@ namespace er {
 void set_last_cuda_error(int e);
 // ER_OK if the current device is compute capability 10.x, ER_ERR_ARCH / ER_ERR_CUDA otherwise.
 int check_arch();
+// Host-side caches (SM count, function attributes, occupancy queries) are kept PER DEVICE, indexed by the
+// cudaGetDevice() id: a process may call the library on several GPUs.
+constexpr int kMaxDevices = 64;
+int current_device();
 int sm_count();
 
 #define ER_CUDA_TRY(expr)                                   \

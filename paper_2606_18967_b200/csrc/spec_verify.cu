@@ -131,7 +131,16 @@ struct ClusterCtx {
   int rank, size;      // this CTA's rank in the cluster, CTAs per cluster
   int tile_lo, tile_hi;  // its range of kTile-token tiles
   int xpar;            // parity of the next exchange buffer
+  bool started;        // the "every CTA of the cluster has started" handshake has been waited for
 };
+
+// A CTA's shared memory may be written remotely only once that CTA has started executing: every CTA arrives
+// (relaxed) on the cluster barrier at kernel entry, and all threads wait for that phase here, right before the
+// first remote store.  Uniform over the CTA; a no-op for clusters of one.
+__device__ __forceinline__ void cluster_started(ClusterCtx& cx) {
+  if (cx.size > 1 && !cx.started) asm volatile("barrier.cluster.wait.aligned;" ::: "memory");
+  cx.started = true;
+}
 
 // Softmax statistics (online max / sum of exponentials) of one target row and (optionally) one draft row over
 // this CTA's tile range, reduced to one entry per warp in sh.wstat[pos].
@@ -165,18 +174,23 @@ __device__ void row_stats(const T* trow, const T* drow, const T* next_t, const T
 #pragma unroll
         for (int i = 1; i < 8; ++i) cm = fmaxf(cm, f[i]);
         if (cm > mt) { st_ *= exp2f((mt - cm) * scale); mt = cm; }
-        const float nt = -mt * scale;
+        if (mt > kNegInf) {   // a chunk of masked (-inf) logits before any finite one adds nothing (and -mt * scale
+                              // would overflow: fma(-inf, scale, +inf) is NaN)
+          const float nt = -mt * scale;
 #pragma unroll
-        for (int i = 0; i < 8; ++i) st_ += ex2_fast(fmaf(f[i], scale, nt));
+          for (int i = 0; i < 8; ++i) st_ += ex2_fast(fmaf(f[i], scale, nt));
+        }
         if (drow) {
           Load8<T>::expand(rd[j], f);
           cm = f[0];
 #pragma unroll
           for (int i = 1; i < 8; ++i) cm = fmaxf(cm, f[i]);
           if (cm > md) { sd_ *= exp2f((md - cm) * scale); md = cm; }
-          const float nd = -md * scale;
+          if (md > kNegInf) {
+            const float nd = -md * scale;
 #pragma unroll
-          for (int i = 0; i < 8; ++i) sd_ += ex2_fast(fmaf(f[i], scale, nd));
+            for (int i = 0; i < 8; ++i) sd_ += ex2_fast(fmaf(f[i], scale, nd));
+          }
         }
       }
     }
@@ -203,6 +217,7 @@ __device__ __forceinline__ void merge_stat(float& m, float& s, float m2, float s
 __device__ void combine_stats(int npos, float scale, Shared& sh, ClusterCtx& cx) {
   const int tid = threadIdx.x;
   cg::cluster_group cluster = cg::this_cluster();
+  cluster_started(cx);
   __syncthreads();
   if (tid < npos) {
     float mt = kNegInf, st = 0.f, md = kNegInf, sd = 0.f;
@@ -307,6 +322,7 @@ __device__ int draw_token(const T* trow, const T* drow, int V, bool vec, float s
   const int par = cx.xpar;
   cx.xpar ^= 1;
   const int nseg = ntile * kWarps;
+  cluster_started(cx);
   if (warp == 0) {
     double mine = 0.0;                       // lane-strided partial sums, then a butterfly: the same value in
     for (int i = lane; i < nseg; i += 32) mine += (double)seg_sums[i];   // every lane, in a fixed order
@@ -412,6 +428,8 @@ spec_verify_kernel(const T* __restrict__ target, const T* __restrict__ draft, fl
   cx.size = (int)cluster.num_blocks();
   cx.rank = (int)cluster.block_rank();
   cx.xpar = 0;
+  cx.started = false;
+  if (cx.size > 1) asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");   // "I have started"
   const int tiles = (V + kTile - 1) / kTile;
   const int per = (tiles + cx.size - 1) / cx.size;
   cx.tile_lo = min(cx.rank * per, tiles);
@@ -502,15 +520,21 @@ int launch_verify(int cluster_size, size_t smem, cudaStream_t s, const T* target
   return ER_OK;
 }
 
-int g_force_cluster = 0;   // sweeps only (er_verify_tuning): 0 = automatic
+#ifdef ER_DEV
+int g_force_cluster = 0;   // development library only (er_dev.h): 0 = automatic
+#else
+constexpr int g_force_cluster = 0;
+#endif
 
 }  // namespace
 
-extern "C" int er_verify_tuning(int cluster) {
+#ifdef ER_DEV
+extern "C" int er_dev_verify_cluster(int cluster) {
   if (cluster != 0 && cluster != 1 && cluster != 2 && cluster != 4 && cluster != 8) return ER_ERR_SHAPE;
   g_force_cluster = cluster;
   return ER_OK;
 }
+#endif
 
 extern "C" int er_spec_verify(const void* target, const void* draft, int in_dtype, int inputs_are_logits,
                               float temperature, const int32_t* draft_tokens, const float* u_accept,

@@ -164,12 +164,38 @@ def test_block_efficiency_matches_paper_table2():
 
 
 def test_widened_interval_rule():
+    # Rule V10, pinned on a hand-built dyadic CDF with R != 1 -- every expectation below is arithmetic
+    # done on paper, none of it comes from the function under test:
+    #   w = (1/4, 0, 1/2, 1/8, 5/8), R = 3/2, C = (1/4, 1/4, 3/4, 7/8, 3/2), C/R = (1/6, 1/6, 1/2, 7/12, 1)
+    # token intervals in units of R: 0:[0,1/6)  1:empty (w = 0)  2:[1/6,1/2)  3:[1/2,7/12)  4:[7/12,1)
+    w = np.array([0.25, 0.0, 0.5, 0.125, 0.625])
+    C = np.array([0.25, 0.25, 0.75, 0.875, 1.5])
+    assert np.array_equal(np.cumsum(w), C)
+    mk = lambda r: {"C": C, "R": 1.5, "w": w, "r": r, "margins": []}
+    # r just above the upper edge of token 2 (the exact token is 3): 0.9e-5 inside the slack, 1.1e-5 outside
+    assert O.token_in_widened_interval(mk(0.5 + 0.9e-5), 2)
+    assert not O.token_in_widened_interval(mk(0.5 + 1.1e-5), 2)
+    # r just below the lower edge of token 3 (the exact token is 2)
+    assert O.token_in_widened_interval(mk(0.5 - 0.9e-5), 3)
+    assert not O.token_in_widened_interval(mk(0.5 - 1.1e-5), 3)
+    # (a missing division by R would put token 3's lower edge at 0.75 and fail the third line; a slack of 1e-1 or
+    #  1e-4 would pass the second and fourth)
+    # a token without mass never passes, even when r sits exactly on its (empty) interval
+    assert not O.token_in_widened_interval(mk(1.0 / 6.0), 1)
+    # the exact token always passes; neighbours far from r do not
+    for r, t in ((0.1, 0), (0.3, 2), (0.55, 3), (0.9, 4)):
+        assert O.token_in_widened_interval(mk(r), t)
+        for other in range(5):
+            if other != t:
+                assert not O.token_in_widened_interval(mk(r), other), (r, t, other)
+    # first token: lower edge is 0 (no C[-1] wrap-around to the total mass)
+    assert O.token_in_widened_interval(mk(0.0), 0) and not O.token_in_widened_interval(mk(0.0), 4)
+    # out-of-range ids
+    assert not O.token_in_widened_interval(mk(0.3), -1) and not O.token_in_widened_interval(mk(0.3), 5)
+    # and through spec_verify's own diagnostics: the oracle's token passes its own window
     p = _probs(1, 2, 10, 7)
     q = _probs(1, 1, 10, 8)
     x = np.array([[0]], np.int32)
     n, out, diag = O.spec_verify(p, q, x, np.array([[0.999]], np.float32), np.array([0.4], np.float32),
                                  inputs_are_logits=False, return_diag=True)
-    t = int(out[0, n[0]])
-    assert O.token_in_widened_interval(diag[0], t)
-    far = (t + 5) % 10
-    assert not O.token_in_widened_interval(diag[0], far) or diag[0]["w"][far] == 0 or abs(far - t) <= 1
+    assert O.token_in_widened_interval(diag[0], int(out[0, n[0]]))
