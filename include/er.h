@@ -129,6 +129,22 @@ int er_w4a16_gemm_simt(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_ele
                        const void* qweight, const void* scales, int64_t N, int group,
                        void* y, int64_t ldy_elems, int y_dtype, void* stream);
 
+/* (1b) bf16 linear  Y[m][n] = sum_k X[m][k] * W[n][k]  with UNQUANTIZED bf16 weights: the drafter's lm_head, which the
+ * paper keeps in higher precision (PAPER.md:L455 sec. D.2 "embedding, LM head, norms"; L101 quantizes only the FFN and
+ * QKVO projections), and the target model's own linears -- the T_p and T_V(gamma) of the paper's speedup model
+ * tau * T_p / (gamma * T_q + T_V) (Eq. 1, L488-L492 Eq. 5).
+ *   x_bf16  [M][K] bf16, row stride ldx_elems; w_bf16 [N][K] bf16 (torch nn.Linear.weight), row stride ldw_elems;
+ *           both bases 16-byte aligned, ldx_elems % 8 == 0, ldw_elems % 8 == 0; M >= 1, N % 128 == 0, K % 128 == 0
+ *   y       [M][N] of y_dtype (ER_F32: the fp32 accumulator; ER_BF16: it rounded RNE), row stride ldy_elems
+ *   workspace  >= er_bf16_gemm_workspace_bytes(M,N,K), 16-byte aligned, its first ER_GEMM_COUNTER_BYTES zero before
+ *           the first use (er_gemm_workspace_init) and left zero by every call; may be shared with er_w4a16_gemm
+ * Arithmetic: bf16 x bf16 products (exact in fp32) accumulated in fp32 on the tensor cores; split-K partials are
+ * reduced in ascending CTA order (deterministic). */
+size_t er_bf16_gemm_workspace_bytes(int64_t M, int64_t N, int64_t K);
+int er_bf16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, const void* w_bf16, int64_t N,
+                 int64_t ldw_elems, void* y, int64_t ldy_elems, int y_dtype, void* workspace, size_t workspace_bytes,
+                 void* stream);
+
 /* (3) Speculative-decoding verification, one result per sequence b < B.
  *   target  [B][gamma+1][V]  (row gamma = bonus position), draft [B][gamma][V]; contiguous, 16-byte aligned
  *   in_dtype / inputs_are_logits: (ER_F32, 0) = fp32 probabilities; (ER_BF16, 1) and (ER_F32, 1) = logits,

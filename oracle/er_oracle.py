@@ -16,10 +16,13 @@ Parity pins (tests/test_oracle_*.py, `-m "not gpu"`):
                   values against exact rational arithmetic, nibble round trip.
   w4a16_gemm      pinned: one-hot read-out, exact-integer probe, pure-Python
                   Fraction brute force on tiny shapes, K-split invariance.
+  bf16_gemm       pinned: pure-Python Fraction brute force, exact-integer case, one-hot read-out.
   spec_verify     pinned: q = p accepts everything, one-hot / zero-probability
                   cases, exact rational enumeration showing the output
                   distribution equals p (the theorem of ref. [29] the paper
                   relies on), scipy softmax.
+  token_in_widened_interval  pinned on a hand-built dyadic CDF with R != 1 (rule V10: edges at
+                  0.9e-5 / 1.1e-5, zero-mass token, first token, out-of-range ids).
   block_efficiency pinned to the values the paper prints (Table 2).
 No function here is "parity unpinned".
 """
@@ -164,6 +167,15 @@ def w4a16_gemm(x_u16: np.ndarray, qweight: np.ndarray, scales_u16: np.ndarray, g
     (a library primitive used as one step, no blocking or reordering of ours)."""
     x = bf16_to_f32(x_u16).astype(np.float64)
     return x @ dequantize(qweight, scales_u16, group).T
+
+
+def bf16_gemm(x_u16: np.ndarray, w_u16: np.ndarray) -> np.ndarray:
+    """y_ref[m][n] = sum_k double(x[m][k]) * double(w[n][k]) with bf16 weights W[N][K] (the drafter's lm_head kept in
+    higher precision; the target model's linears behind T_p / T_V of Eq. 1).
+    The definition written out; numpy's fp64 matmul is the library primitive used as the one step."""
+    x = bf16_to_f32(x_u16).astype(np.float64)
+    w = bf16_to_f32(w_u16).astype(np.float64)
+    return x @ w.T
 
 
 # ----------------------------------------------------------------------------

@@ -64,7 +64,7 @@ __device__ __forceinline__ uint32_t code_bits_div(float w, float s) {  // denorm
   return __float_as_uint(__fdiv_rn(w, s) + kMagic);
 }
 
-// Packs the 8 codes of 4 raw words (k = 0..7 of the word) into one ER_PACK_V1 word: logical k = 2 t + h sits in
+// Packs the 8 codes of 4 raw words (k = 0..7 of the word) into one packed word (ER_PACK_V2 keeps this intra-word order): logical k = 2 t + h sits in
 // nibble t + 4 h.  `sum of (0x4B400000 << 4 i)` over i = 0..7 (mod 2^32) is the constant removed at the end.
 template <bool kDiv>
 __device__ __forceinline__ uint32_t pack8(const uint32_t* raw, float s, float r) {
@@ -155,6 +155,13 @@ __device__ __forceinline__ void quantize_tile(const uint16_t* __restrict__ w, in
     const int64_t gg = ((int64_t)bx * kTileK >> 7) + g, n = n0 + r;
     if (n < N && gg < (K >> 7)) scales[gg * N + n] = s_scales[g][r];
   }
+  // The refresh is immediately followed by drafter GEMMs that are launched with programmatic stream serialization and
+  // that start streaming the packed weights BEFORE their griddepcontrol.wait (w4a16_gemm_small.cu).  They may do so
+  // only once every CTA of this kernel has passed this point: the CTA's stores are made visible device-wide (also to
+  // the async proxy the bulk copies read through), then the dependent launch is allowed.
+  __threadfence();
+  asm volatile("fence.proxy.async;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 
 __global__ void __launch_bounds__(kThreads) quantize_pack_kernel(const uint16_t* __restrict__ w, int64_t N,

@@ -6,8 +6,8 @@ call returns a non-zero status, an exception is raised.
 """
 from __future__ import annotations
 
+import contextlib
 import ctypes
-import os
 
 import torch
 
@@ -35,15 +35,8 @@ class ErError(RuntimeError):
         self.status = status
 
 
-def load() -> ctypes.CDLL:
-    """Load (building first if stale/missing) the C-ABI library.  Raises if it cannot be had."""
-    global _lib
-    if _lib is not None:
-        return _lib
-    path = _build.LIB_PATH
-    if not os.path.exists(path) or (os.environ.get("ER_REBUILD") == "1"):
-        path = _build.build_library()
-    lib = ctypes.CDLL(path)
+def _bind(lib: ctypes.CDLL) -> ctypes.CDLL:
+    """Declare the argument / result types of every entry point of include/er.h."""
     vp, i64, i32, sz, f32 = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int32, ctypes.c_size_t, ctypes.c_float
     lib.er_status_str.restype = ctypes.c_char_p
     lib.er_status_str.argtypes = [ctypes.c_int]
@@ -65,6 +58,10 @@ def load() -> ctypes.CDLL:
     lib.er_w4a16_gemm.argtypes = [vp, i64, i64, i64, vp, vp, i64, ctypes.c_int, vp, i64, ctypes.c_int, vp, sz, vp]
     lib.er_w4a16_gemm_simt.restype = ctypes.c_int
     lib.er_w4a16_gemm_simt.argtypes = [vp, i64, i64, i64, vp, vp, i64, ctypes.c_int, vp, i64, ctypes.c_int, vp]
+    lib.er_bf16_gemm_workspace_bytes.restype = sz
+    lib.er_bf16_gemm_workspace_bytes.argtypes = [i64, i64, i64]
+    lib.er_bf16_gemm.restype = ctypes.c_int
+    lib.er_bf16_gemm.argtypes = [vp, i64, i64, i64, vp, i64, i64, vp, i64, ctypes.c_int, vp, sz, vp]
     lib.er_spec_verify.restype = ctypes.c_int
     lib.er_spec_verify.argtypes = [vp, vp, ctypes.c_int, ctypes.c_int, f32, vp, vp, vp, i32, i32, i32, vp, vp, vp]
     lib.er_unpack_codes.restype = ctypes.c_int
@@ -82,12 +79,40 @@ def load() -> ctypes.CDLL:
     lib.er_spec_verify_host.restype = ctypes.c_int
     lib.er_spec_verify_host.argtypes = [vp, vp, ctypes.c_int, ctypes.c_int, f32, vp, vp, vp, i32, i32, i32, vp, vp, vp,
                                         sz, vp]
-    lib.er_gemm_tuning.restype = ctypes.c_int
-    lib.er_gemm_tuning.argtypes = [ctypes.c_int, ctypes.c_int]
     if lib.er_abi_version() != 1:
         raise RuntimeError("liber_b200.so ABI version mismatch")
-    _lib = lib
     return lib
+
+
+def load() -> ctypes.CDLL:
+    """Load the C-ABI library, (re)building it first when it is missing or older than its sources
+    (build_library is a no-op when the .so is fresh).  Raises if it cannot be had: there is no other path."""
+    global _lib
+    if _lib is None:
+        _lib = _bind(ctypes.CDLL(_build.build_library()))
+    return _lib
+
+
+@contextlib.contextmanager
+def dev_library():
+    """Tests only: route this module's calls through the DEVELOPMENT build (liber_b200_dev.so, csrc/er_dev.h), which
+    adds the partition / launch-mode knobs, and hand the library out so that they can be set.  Every knob is reset
+    and the shipped library restored on exit."""
+    global _lib
+    lib = _bind(ctypes.CDLL(_build.build_library(dev=True)))
+    lib.er_dev_gemm_tuning.restype = ctypes.c_int
+    lib.er_dev_gemm_tuning.argtypes = [ctypes.c_int, ctypes.c_int]
+    lib.er_dev_verify_cluster.restype = ctypes.c_int
+    lib.er_dev_verify_cluster.argtypes = [ctypes.c_int]
+    prev = load()
+    _lib = lib
+    try:
+        yield lib
+    finally:
+        for key, value in ((1, 0), (3, 1), (4, 1), (5, 1), (6, 1)):
+            lib.er_dev_gemm_tuning(key, value)
+        lib.er_dev_verify_cluster(0)
+        _lib = prev
 
 
 def _stream(t: torch.Tensor) -> int:
@@ -128,7 +153,7 @@ def gemm_workspace(M: int, N: int, K: int, device) -> torch.Tensor:
 
 def quantize_pack(w: torch.Tensor, qweight: torch.Tensor | None = None, scales: torch.Tensor | None = None,
                   group: int = GROUP):
-    """bf16 W[N][K] -> (qweight int32 [N][K/8] (ER_PACK_V1 bits), scales bf16 [K/128][N])."""
+    """bf16 W[N][K] -> (qweight int32 [N][K/8] (ER_PACK_V2 layout, include/er.h), scales bf16 [K/128][N])."""
     _cuda(w, "w")
     assert w.dtype == torch.bfloat16 and w.dim() == 2 and w.stride(1) == 1
     N, K = w.shape
@@ -175,6 +200,28 @@ def w4a16_gemm(x: torch.Tensor, qweight: torch.Tensor, scales: torch.Tensor, out
     _check(lib.er_w4a16_gemm(x.data_ptr(), M, K, x.stride(0), qweight.data_ptr(), scales.data_ptr(), N, GROUP,
                              y.data_ptr(), y.stride(0), ydt, workspace.data_ptr(), workspace.numel(), _stream(x)),
            "er_w4a16_gemm")
+    return y
+
+
+def bf16_gemm(x: torch.Tensor, w: torch.Tensor, out_dtype=torch.bfloat16, y: torch.Tensor | None = None,
+              workspace: torch.Tensor | None = None):
+    """Y[M][N] = X[M][K] . W[N][K]^T with bf16 weights (lm_head, target-side linears)."""
+    _cuda(x, "x")
+    assert x.dtype == torch.bfloat16 and w.dtype == torch.bfloat16 and x.stride(1) == 1 and w.stride(1) == 1
+    M, K = x.shape
+    N = w.shape[0]
+    if y is None:
+        y = torch.empty((M, N), dtype=out_dtype, device=x.device)
+    ydt = ER_F32 if y.dtype == torch.float32 else ER_BF16
+    lib = load()
+    if workspace is None:
+        nbytes = lib.er_bf16_gemm_workspace_bytes(M, N, K)
+        if nbytes == 0:
+            raise ErError(2, "er_bf16_gemm_workspace_bytes")
+        workspace = torch.empty(nbytes, dtype=torch.uint8, device=x.device)
+        _check(lib.er_gemm_workspace_init(workspace.data_ptr(), nbytes, _stream(x)), "er_gemm_workspace_init")
+    _check(lib.er_bf16_gemm(x.data_ptr(), M, K, x.stride(0), w.data_ptr(), N, w.stride(0), y.data_ptr(), y.stride(0), ydt,
+                            workspace.data_ptr(), workspace.numel(), _stream(x)), "er_bf16_gemm")
     return y
 
 

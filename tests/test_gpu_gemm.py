@@ -125,18 +125,18 @@ def test_split_k_counts_agree_and_are_deterministic(splits):
     qw, sc = _dev_weights(codes, su)
     rng = np.random.default_rng(1)
     x = torch.from_numpy(rng.integers(-1, 3, size=(M, K)).astype(np.float32)).to(DEV).to(torch.bfloat16)
-    lib = er.load()
-    try:
-        assert lib.er_gemm_tuning(1, splits) == 0
-        ws = er.gemm_workspace(M, N, K, DEV)
-        y1 = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32, workspace=ws)
-        y2 = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32, workspace=ws)   # workspace reuse: counters self-reset
-        torch.cuda.synchronize()
-    finally:
-        lib.er_gemm_tuning(1, 0)
-    ref = O.w4a16_gemm(I.as_u16(x), qw.cpu().numpy().view(np.uint32), su)
-    assert np.array_equal(y1.cpu().numpy().astype(np.float64), ref)
-    assert torch.equal(y1, y2)
+    for small in (1, 0):                                 # M <= 8 would take the warp-level-MMA kernel: both kernels
+        with er.dev_library() as lib:
+            assert lib.er_dev_gemm_tuning(1, splits) == 0
+            assert lib.er_dev_gemm_tuning(6, small) == 0
+            ws = er.gemm_workspace(M, N, K, DEV)
+            for Mx in (M, 8):
+                y1 = er.w4a16_gemm(x[:Mx], qw, sc, out_dtype=torch.float32, workspace=ws)
+                y2 = er.w4a16_gemm(x[:Mx], qw, sc, out_dtype=torch.float32, workspace=ws)   # workspace reuse: counters self-reset
+                torch.cuda.synchronize()
+                ref = O.w4a16_gemm(I.as_u16(x[:Mx]), qw.cpu().numpy().view(np.uint32), su)
+                assert np.array_equal(y1.cpu().numpy().astype(np.float64), ref), (small, Mx)
+                assert torch.equal(y1, y2)
 
 
 def _sampled_columns_check(x, qw, sc, N, K, seed, label, y=None):
@@ -157,13 +157,23 @@ def _sampled_columns_check(x, qw, sc, N, K, seed, label, y=None):
     got = y[:, ct].cpu().numpy().astype(np.float64)
     err = np.abs(got - y_ref).max()
     assert err <= _tol(y_ref), f"{label} M={M}: max|d|={err} tol={_tol(y_ref)}"
+    # ALL N columns: the tensor-core kernel against the plain CUDA-core kernel (same contract, different summation
+    # order), which is itself pinned to the oracle on the sampled tiles -- stream-K range boundaries fall in different
+    # places in every tile, so the sample alone would not see a mistake there
+    y_simt = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32, simt=True)
+    torch.cuda.synchronize()
+    err_s = np.abs(y_simt[:, ct].cpu().numpy().astype(np.float64) - y_ref).max()
+    assert err_s <= _tol(y_ref), f"{label} M={M}: SIMT max|d|={err_s}"
+    rms = float(y_simt.float().pow(2).mean().sqrt())
+    gap = float((y - y_simt).abs().max())
+    assert gap <= 1e-4 * rms + 1e-5, f"{label} M={M}: tcgen05 vs SIMT over all columns: {gap} (rms {rms})"
     assert torch.isfinite(y).all()
     return y
 
 
 @pytest.mark.parametrize("name,N,K", [("qkv", 4608, 3584), ("o", 3584, 3584), ("gate_up", 37888, 3584),
                                       ("down", 3584, 18944)])
-@pytest.mark.parametrize("M", [1, 16, 256])
+@pytest.mark.parametrize("M", [1, 8, 16, 256])
 def test_config1_full_size_sampled_columns(name, N, K, M):
     # full 7B-layer shapes in the launch configuration bench.py times
     w = I.weight_bf16(N, K, I.seed_of("cfg1", name), device=DEV)
@@ -227,18 +237,48 @@ def test_programmatic_dependent_launch_does_not_change_results():
     qw, sc = er.quantize_pack(w)
     x0 = I.activation_bf16(M, K, I.seed_of("pdl", "x"), device=DEV)
     ws = er.gemm_workspace(M, N, K, DEV)
-    lib = er.load()
     outs = []
-    for pdl in (1, 0):
-        assert lib.er_gemm_tuning(3, pdl) == 0
-        x = x0
-        for _ in range(4):          # y feeds the next call: a chain of dependent launches
-            y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.bfloat16, workspace=ws)
-            x = (y.float() / y.float().pow(2).mean().sqrt()).to(torch.bfloat16)
-        torch.cuda.synchronize()
-        outs.append(y.clone())
-    lib.er_gemm_tuning(3, 1)
+    with er.dev_library() as lib:
+        for pdl in (1, 0):
+            assert lib.er_dev_gemm_tuning(3, pdl) == 0
+            x = x0
+            for _ in range(4):          # y feeds the next call: a chain of dependent launches
+                y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.bfloat16, workspace=ws)
+                x = (y.float() / y.float().pow(2).mean().sqrt()).to(torch.bfloat16)
+            torch.cuda.synchronize()
+            outs.append(y.clone())
     assert torch.equal(outs[0], outs[1])
+    # ... and the shipped library gives those bits too
+    x = x0
+    for _ in range(4):
+        y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.bfloat16, workspace=ws)
+        x = (y.float() / y.float().pow(2).mean().sqrt()).to(torch.bfloat16)
+    torch.cuda.synchronize()
+    assert torch.equal(y, outs[0])
+
+
+def test_refresh_then_gemm_back_to_back_sees_the_new_weights():
+    # er_quantize_pack immediately followed by er_w4a16_gemm on the same stream, repeatedly with DIFFERENT weights in
+    # the same buffers (the per-RL-step refresh): the GEMM (programmatic dependent launch; the M <= 8
+    # kernel even starts streaming weights before its griddepcontrol.wait) must never read stale packed words
+    N, K = 37888, 3584
+    qw = torch.empty((N, K // 8), dtype=torch.int32, device=DEV)
+    sc = torch.empty((K // 128, N), dtype=torch.bfloat16, device=DEV)
+    ws = er.gemm_workspace(16, N, K, DEV)
+    for M in (4, 16):
+        x = I.activation_bf16(M, K, I.seed_of("b2b", "x", M), device=DEV)
+        ws_ = [I.weight_bf16(N, K, I.seed_of("b2b", r), device=DEV) for r in range(3)]
+        ys = []
+        for r in range(3):
+            er.quantize_pack(ws_[r], qw, sc)
+            ys.append(er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32, workspace=ws))
+        torch.cuda.synchronize()
+        for r in range(3):               # the same, with a device synchronisation between refresh and GEMM
+            er.quantize_pack(ws_[r], qw, sc)
+            torch.cuda.synchronize()
+            y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32, workspace=ws)
+            torch.cuda.synchronize()
+            assert torch.equal(y, ys[r]), (M, r)
 
 
 @pytest.mark.parametrize("mode", ["cluster", "tile_split", "stream_k"])
@@ -249,17 +289,34 @@ def test_partition_modes_agree_with_the_oracle_and_are_deterministic(mode):
     w = I.weight_bf16(N, K, I.seed_of("modes", "w"), device=DEV)
     x = I.activation_bf16(M, K, I.seed_of("modes", "x"), device=DEV)
     qw, sc = er.quantize_pack(w)
-    lib = er.load()
-    lib.er_gemm_tuning(5, 1 if mode == "cluster" else 0)
-    lib.er_gemm_tuning(4, 0 if mode == "stream_k" else 1)
-    try:
-        y1 = _sampled_columns_check(x, qw, sc, N, K, 7, mode)
-        y2 = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
-        torch.cuda.synchronize()
-        assert torch.equal(y1, y2)
-    finally:
-        lib.er_gemm_tuning(5, 1)
-        lib.er_gemm_tuning(4, 1)
+    with er.dev_library() as lib:
+        lib.er_dev_gemm_tuning(5, 1 if mode == "cluster" else 0)
+        lib.er_dev_gemm_tuning(4, 0 if mode == "stream_k" else 1)
+        for Mx in (M, 8, 3):          # M <= 8 without a cluster goes through the warp-level-MMA kernel
+            y1 = _sampled_columns_check(x[:Mx], qw, sc, N, K, 7, mode)
+            y2 = er.w4a16_gemm(x[:Mx], qw, sc, out_dtype=torch.float32)
+            torch.cuda.synchronize()
+            assert torch.equal(y1, y2)
+
+
+@pytest.mark.parametrize("M", [1, 5, 8])
+def test_both_small_batch_kernels_agree_with_the_oracle(M):
+    # M <= 8 on a plan without a cluster runs the warp-level-MMA kernel (w4a16_gemm_small.cu); the development
+    # library can send the same problem through the tcgen05 kernel: both against the oracle, on a shape with whole
+    # tiles and partial tiles per CTA (stream-K) and on a raw-nibble matrix that contains the code -8
+    for N, K in ((37888, 3584), (1024, 1152)):
+        codes = I.random_codes(N, K, N + M) if N == 1024 else None
+        if codes is None:
+            w = I.weight_bf16(N, K, I.seed_of("small", N), device=DEV)
+            qw, sc = er.quantize_pack(w)
+            del w
+        else:
+            qw, sc = _dev_weights(codes, _random_scales(K // 128, N, 5))
+        x = I.activation_bf16(M, K, I.seed_of("small", "x", M), device=DEV)
+        with er.dev_library() as lib:
+            for small in (1, 0):
+                lib.er_dev_gemm_tuning(6, small)
+                _sampled_columns_check(x, qw, sc, N, K, N + M + small, f"small_mma={small}")
 
 
 @pytest.mark.parametrize("M", [1, 16, 64])
