@@ -1,31 +1,39 @@
-// w4a16_gemm_small.cu -- er_w4a16_gemm at M <= 16: the memory-bound regime of the weight-quantized self-drafter
-// ("weight loading dominates" small-batch decode; L175 W4A16 weight-only kernel; L467 "on-the-fly
-// dequantization and kernel-level overhead" is what eta_D pays on top of the bytes).
+// w4a16_gemm_small.cu -- er_w4a16_gemm at M <= 8 on plans without a thread-block cluster (the large-N linears, e.g.
+// gate/up): the most memory-bound corner of the weight-quantized self-drafter ("weight loading dominates"
+// small-batch decode; L175 W4A16 weight-only kernel; L467 "on-the-fly dequantization and kernel-level overhead" is
+// what eta_D pays on top of the bytes).
 //
-// What bounds this regime on sm_100a is not the contraction (2 * 16 * 128 * 128 flop per 8 KiB of weights, 3 % of
-// the tensor peak) but (a) the nibble -> bf16 conversion, 7 half-rate logic-pipe operations per packed word = 224
-// ALU cycles per [128 rows x 128 k] block and SM sub-partition against 370 cycles of HBM time, and (b) whatever
-// the warps have to wait for.  The tcgen05 form of this kernel (w4a16_gemm.cu, still used for M > 16) needs a
-// CTA-wide rendezvous per 128-k group twice -- all 128 rows of the A operand in TENSOR MEMORY before the MMA, the
-// accumulator read back after it for the exact per-group scale -- and measured 600 cycles per group with the
-// logic pipe 50 % idle (profiles/r02_*).  Here every warp is on its own:
+// What bounds this regime on sm_100a is not the contraction (2 * 8 * 128 * 128 flop per 8 KiB of weights) but the
+// nibble -> bf16 conversion -- 7 half-rate logic-pipe operations per packed word = 224 ALU cycles per [128 rows x 128
+// k] block and SM sub-partition against 370 cycles of HBM time -- and whatever the warps have to wait for.  The
+// tcgen05 kernel (w4a16_gemm.cu) needs a CTA-wide rendezvous per 128-k group twice (all 128 rows of the A operand in
+// TENSOR MEMORY before the MMA, the accumulator read back after it for the exact per-group scale).  Here every warp
+// is on its own; measured on gate/up at M <= 8: 16.9 us against 18.5-19.0 us (profiles/r02_gemm.md, which also has
+// the experiments behind every choice below).
 //
 //   persistent   one CTA per SM; the (tile, 128-k group) units are dealt out as one contiguous range per CTA
-//                (stream-K / tile split / thread-block cluster, w4a16_plan.cuh), as in the tcgen05 kernel.
-//   warp 20      producer: per group ONE 8 KiB bulk copy of the packed block (ER_PACK_V2), 256 B of scales and two
-//                SWIZZLE_128B TMA boxes of X, into a ring of up to 12 stages; full / empty mbarriers.
+//                (stream-K / tile split, w4a16_plan.cuh), as in the tcgen05 kernel.
+//   two rings    packed weights (8 KiB stages, up to 20) and X + scales + x sums (3 KiB stages, 10).  A weight stage
+//                is handed back as soon as its words sit in registers, at the START of a group's contraction, so the
+//                weight ring is almost entirely bytes in flight.
+//   warp 20      weight producer: one 8 KiB 1-D bulk copy per group (ER_PACK_V2 keeps the block contiguous and
+//                pre-swizzled).  It does not wait for the previous kernel (griddepcontrol.wait): the weights never
+//                depend on it (include/er.h "Ordering").
+//   warps 21-25  one X warp per worker set: loads the X boxes and the scales of the set's groups and, when they have
+//                landed, sums x[m][k] over the group's 128 k with the tensor cores (A = ones) -- the 136 * sum that
+//                the stored nibble's offset adds to every output of the group (one helper warp for all groups was the
+//                bottleneck of an earlier version: ~350 cycles of dependent latency per group).
 //   warps 0-19   five sets of four warps; set j takes the groups j, j + 5, ... of the CTA's range.  A warp owns 32
 //                weight rows of the group (two 16-row blocks) and all 128 k: 4 x LDS.128 of packed words, nibble
-//                -> bf16 in registers ((w >> 4t) & 0x000F000F | 0x43004300 = 128 + u, one packed fma removes the
-//                136), and mma.sync.m16n8k16 (bf16 x bf16 -> fp32) with the weights as the A fragment and X as the
-//                B fragment: the swap-AB of the tcgen05 kernel at warp level, a batch of 8 / 16 rows is one / two
-//                n8 blocks.  The k index of an MMA is only a label: thread t of a quad takes the k = 32 t .. 32 t + 31
-//                of a row, i.e. exactly one 16-byte chunk of ER_PACK_V2, and reads the matching 64 bytes of X.
-//                The group's fp32 sum is multiplied by the group scale and added to the running sum (no rounding
-//                of q * s).  No warp ever waits for another one inside the main loop.
+//                -> bf16 in registers ((w >> 4t) & 0x000F000F | 0x43004300 = 128 + u), and mma.sync.m16n8k16 (bf16 x
+//                bf16 -> fp32) with the weights as the A fragment and X as the B fragment: the swap-AB of the tcgen05
+//                kernel at warp level.  The k index of an MMA is only a label: thread t of a quad takes the k = 32 t
+//                .. 32 t + 31 of a row, i.e. exactly one 16-byte chunk of ER_PACK_V2, and reads the matching 64 bytes
+//                of X.  The group's fp32 sum, minus 136 * sum x, is multiplied by the group scale and added to the
+//                running sum (no rounding of q * s).  No warp waits for another one inside the main loop.
 //   output       at the end of a tile segment the five sets add their sums in set order through one shared-memory
 //                tile; whole tiles are stored directly, partial ones go through the workspace (ticket per tile,
-//                ascending CTA order) or, in cluster mode, through distributed shared memory.  Deterministic.
+//                ascending CTA order).  Deterministic.
 #include "w4a16_plan.cuh"
 
 namespace {
@@ -36,11 +44,10 @@ constexpr int kSets = 5;
 constexpr int kSetWarps = 4;
 constexpr int kSetThreads = kSetWarps * 32;          // 128
 constexpr int kWorkerWarps = kSets * kSetWarps;      // 20
-constexpr int kProdWarp = kWorkerWarps;              // 12: the weight producer; warps 13 .. 15: one X warp per set
-constexpr int kThreads = (kWorkerWarps + 1 + kSets) * 32;   // 512
-constexpr int kXStages = 10;                         // ring of X / scale stages: the five groups being contracted + 10 ahead
+constexpr int kProdWarp = kWorkerWarps;              // 20: the weight producer; warps 21 .. 25: one X warp per set
+constexpr int kThreads = (kWorkerWarps + 1 + kSets) * 32;   // 832
+constexpr int kXStages = 10;                         // ring of X / scale stages: two per set
 constexpr int kMaxWStages = 20;                      // ring of packed-weight stages: as deep as shared memory allows
-constexpr int kSmemHalf = 113 * 1024;                  // two CTAs (of consecutive launches) share an SM
 constexpr int kRedLd = 132;                          // row pitch of the shared reduction tile (bank-conflict free)
 
 template <int MB>
@@ -49,8 +56,8 @@ struct SCfg {
   // TWO rings.  A packed-weight stage (8 KiB) is handed back as soon as its words sit in registers, at the START of
   // a group's contraction, so that nearly the whole weight ring is bytes in flight: the HBM stream needs about 100
   // KB outstanding per SM (6.4 TB/s x 2.3 us / 148), and a single ring whose stages stay occupied until the group is
-  // contracted never gets there (measured: 4.5 TB/s with 12 stages of which 5 are being worked on).  X, the scales and
-  // the x sums of a group live in the small second ring until the group is finished.
+  // contracted never gets there.  X, the scales and the x sums of a group live in the small second ring until the
+  // group is finished.
   // X of a group: k 0..63 as a box of MPAD rows, k 64..127 as a box of MPAD + 2 rows that starts two rows EARLIER
   // (rows -2, -1 are out of bounds and arrive as zeros): the 128-byte swizzle then differs between the boxes by 2,
   // and the eight lanes of a quarter-warp (rows g, g + 1, four 64-byte column blocks) hit eight different 16-byte

@@ -27,6 +27,35 @@ def test_library_loads_and_exports_every_declared_symbol():
     assert lib.er_abi_version() == 1
 
 
+def _exported(path):
+    import subprocess
+    out = subprocess.run(["nm", "-D", "--defined-only", path], check=True, capture_output=True, text=True).stdout
+    return sorted({ln.split()[-1] for ln in out.splitlines() if " T " in ln and ln.split()[-1].startswith("er_")})
+
+
+def test_export_list_equals_the_header_both_directions():
+    # the shipped library exports exactly what include/er.h declares -- no tuning hooks, no debug entry
+    # points; the development knobs (csrc/er_dev.h) exist only in liber_b200_dev.so
+    from paper_2606_18967_b200 import build
+    assert _exported(build.build_library()) == _declared_symbols()
+    dev = set(_exported(build.build_library(dev=True)))
+    assert dev - set(_declared_symbols()) == {"er_dev_gemm_tuning", "er_dev_verify_cluster"}
+
+
+def test_bf16_gemm_validation():
+    lib = er.load()
+    buf = (ctypes.c_uint8 * 4096)()
+    p = (ctypes.addressof(buf) + 15) & ~15
+    big = 1 << 30
+    assert lib.er_bf16_gemm(None, 1, 128, 128, p, 128, 128, p, 128, 0, p, big, None) == 1
+    assert lib.er_bf16_gemm(p, 1, 128, 128, p, 100, 128, p, 128, 0, p, big, None) == 2
+    assert lib.er_bf16_gemm(p, 1, 128, 128, p, 128, 64, p, 128, 0, p, big, None) == 2      # ldw < K
+    assert lib.er_bf16_gemm(p, 1, 128, 128, p, 128, 128, p, 128, 7, p, big, None) == 4
+    assert lib.er_bf16_gemm(p + 2, 1, 128, 128, p, 128, 128, p, 128, 0, p, big, None) == 3
+    assert lib.er_bf16_gemm(p, 1, 128, 128, p, 128, 128, p, 128, 0, p, 16, None) == 5
+    assert lib.er_bf16_gemm_workspace_bytes(1, 128, 128) >= er.COUNTER_BYTES
+
+
 def test_status_strings():
     lib = er.load()
     assert lib.er_status_str(0) == b"ER_OK"

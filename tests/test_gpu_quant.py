@@ -108,3 +108,67 @@ def test_batched_equals_separate_calls():
     torch.cuda.synchronize()
     for (w, q2, s2), (q1, s1) in zip(items, refs):
         assert torch.equal(q1, q2) and torch.equal(s1.view(torch.int16), s2.view(torch.int16))
+
+
+def test_every_positive_finite_bf16_value_as_group_maximum():
+    # DESIGN.md Q4: the kernel computes s = bf16_rne(amax * (1/7)); the reading is IEEE division.  There are only 32 640
+    # positive finite bf16 values: each one is the maximum of one group here, and the stored scale bits (and codes) must
+    # equal the oracle's, which divides.  (255 row tiles of 128 rows x one group.)
+    amax = np.arange(0x0001, 0x7F80, dtype=np.uint16)          # every positive finite bf16, denormals included
+    assert len(amax) == 0x7F80 - 1
+    n = ((len(amax) + 127) // 128) * 128
+    a = np.concatenate([amax, np.full(n - len(amax), 0x3F80, dtype=np.uint16)])
+    rng = np.random.default_rng(11)
+    w = np.zeros((n, 128), dtype=np.uint16)
+    w[:, 0] = a ^ (rng.integers(0, 2, size=n).astype(np.uint16) << 15)          # random sign
+    # the rest of the group: random fractions of the maximum (same exponent range), so codes are exercised as well
+    frac = rng.random((n, 127), dtype=np.float32) * 2 - 1
+    rest = O.f32_to_bf16_rne((O.bf16_to_f32(a)[:, None] * frac).astype(np.float32))
+    w[:, 1:] = rest
+    wt = I.from_u16(w, DEV)
+    qw, sc = er.quantize_pack(wt)
+    torch.cuda.synchronize()
+    codes_ref, sr = O.quantize_codes(w)
+    assert np.array_equal(I.as_u16(sc), sr), "scale bits differ from the IEEE division for some amax"
+    assert np.array_equal(er.unpack_codes(qw).cpu().numpy(), codes_ref)
+
+
+def test_config3_layer0_all_four_linears_bit_exact():
+    # BASELINE.json configs[3]: "fully on layer 0" -- packed words and scales of QKV, O, gate/up and down of layer 0
+    # (233 M parameters, N(0, 0.02) with 0.1 % outliers at 20x) byte-compared with the oracle, in row chunks so that the
+    # numpy oracle stays within a few GB
+    for name, N, K in I.SHAPE_7B.linears():
+        w = I.weight_bf16(N, K, I.seed_of("cfg3", 0, name), device=DEV, outlier_frac=0.001)
+        qw, sc = er.quantize_pack(w)
+        torch.cuda.synchronize()
+        G = K // 128
+        qw_np = qw.cpu().numpy().view(np.uint32).reshape(-1)
+        sc_np = I.as_u16(sc)
+        chunk = 2048 if K <= 4096 else 512
+        for r0 in range(0, N, chunk):
+            r1 = min(N, r0 + chunk)
+            qr, sr = O.quantize_pack(I.as_u16(w[r0:r1]))
+            assert np.array_equal(qw_np[(r0 // 128) * G * 2048:(r1 // 128) * G * 2048], qr.reshape(-1)), (name, r0)
+            assert np.array_equal(sc_np[:, r0:r1], sr), (name, r0)
+        del w, qw, sc
+
+
+@pytest.mark.parametrize("layer", [1, 9, 18, 27])
+def test_config3_other_layers_sampled_one_percent_of_groups(layer):
+    # the remaining layers: a seeded 1 % of the (row, group) pairs of every linear against the oracle
+    for name, N, K in I.SHAPE_7B.linears():
+        w = I.weight_bf16(N, K, I.seed_of("cfg3", layer, name), device=DEV, outlier_frac=0.001)
+        qw, sc = er.quantize_pack(w)
+        codes = er.unpack_codes(qw)
+        torch.cuda.synchronize()
+        G = K // 128
+        rng = np.random.default_rng(I.seed_of("cfg3", "sample", layer, name))
+        pick = np.sort(rng.choice(N * G, size=max(1, N * G // 100), replace=False))
+        rows, groups = pick // G, pick % G
+        rt, gt = torch.from_numpy(rows).to(DEV), torch.from_numpy(groups).to(DEV)
+        kk = gt[:, None] * 128 + torch.arange(128, device=DEV)[None, :]
+        wg = w[rt[:, None], kk].contiguous()                       # [n_pick][128]: one group per row
+        cref, sref = O.quantize_codes(I.as_u16(wg))                # scales [1][n_pick]
+        assert np.array_equal(codes[rt[:, None], kk].cpu().numpy(), cref), (layer, name)
+        assert np.array_equal(I.as_u16(sc[gt, rt].contiguous().view(1, -1)), sref), (layer, name)
+        del w, qw, sc, codes

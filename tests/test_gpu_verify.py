@@ -107,6 +107,86 @@ def test_config4_bf16_logits(gamma):
     assert n_exact >= B // 2   # most tokens are exactly the oracle's; the rest passed the V10 window
 
 
+def _device_workload(B, gamma, V, tag):
+    """Config-4 verify inputs generated on the device (the numpy generators need minutes at B = 64-256); both sides
+    see the same bf16 bytes."""
+    tgt, drf = I.verify_logits_bf16_device(B, gamma, V, I.seed_of(tag, "logits", B, gamma), DEV)
+    toks = I.sample_draft_tokens_gumbel(drf, I.seed_of(tag, "tok", B, gamma))
+    ua = I.uniforms((B, gamma), I.seed_of(tag, "ua", B, gamma))
+    us = I.uniforms((B,), I.seed_of(tag, "us", B, gamma))
+    return tgt, drf, toks, ua, us
+
+
+def _check_against_oracle(tgt, drf, toks, ua, us, acc, out, rows=None):
+    """acc / out from the device for ALL sequences; the oracle on `rows` (default all)."""
+    B, G1, V = tgt.shape
+    rows = list(range(B)) if rows is None else rows
+    acc, out = acc.cpu().numpy(), out.cpu().numpy()
+    toks_h = toks.cpu().numpy()
+    n_exact = 0
+    for b in rows:
+        a_ref, o_ref, diag = O.spec_verify(tgt[b:b + 1].float().cpu().numpy(), drf[b:b + 1].float().cpu().numpy(),
+                                           toks_h[b:b + 1], ua[b:b + 1], us[b:b + 1], inputs_are_logits=True,
+                                           return_diag=True)
+        thin = [m for m in diag[0]["margins"] if m < 1e-5]
+        assert not thin, f"sequence {b}: accept test with margin < 1e-5 (listed, never re-seeded): {thin}"
+        n = int(a_ref[0])
+        assert acc[b] == n, (b, acc[b], n)
+        assert np.array_equal(out[b, :n], o_ref[0, :n]) and np.all(out[b, n + 1:] == -1)
+        if out[b, n] == o_ref[0, n]:
+            n_exact += 1
+        else:
+            assert O.token_in_widened_interval(diag[0], int(out[b, n])), (b, out[b, n], o_ref[0, n])
+    return n_exact
+
+
+@pytest.mark.parametrize("gamma", [2, 4, 8])
+def test_config4_full_batch_64(gamma):
+    # BASELINE.json configs[4] as stated: batch 64, vocab 152064, bf16 logits, draft = target + N(0, 0.5^2)
+    B, V = 64, 152064
+    tgt, drf, toks, ua, us = _device_workload(B, gamma, V, "cfg4full")
+    acc, out = er.spec_verify(tgt, drf, toks, torch.from_numpy(ua).to(DEV), torch.from_numpy(us).to(DEV), True)
+    torch.cuda.synchronize()
+    n_exact = _check_against_oracle(tgt, drf, toks, ua, us, acc, out)
+    assert n_exact >= B // 2
+    assert 0.5 * gamma <= float(acc.float().mean()) <= gamma      # alpha ~ 0.8 (SURVEY.md App. B)
+
+
+def test_config2_maximum_batch_256_gamma_8():
+    # config 2's largest verify (B = M = 256, gamma = 8): 2048 CTAs in clusters of 8, several residency waves; every
+    # sequence's structural properties + the oracle on a seeded quarter of the sequences
+    B, gamma, V = 256, 8, 152064
+    tgt, drf, toks, ua, us = _device_workload(B, gamma, V, "cfg2max")
+    acc, out = er.spec_verify(tgt, drf, toks, torch.from_numpy(ua).to(DEV), torch.from_numpy(us).to(DEV), True)
+    torch.cuda.synchronize()
+    a, o, t = acc.cpu().numpy(), out.cpu().numpy(), toks.cpu().numpy()
+    for b in range(B):
+        n = int(a[b])
+        assert 0 <= n <= gamma and np.array_equal(o[b, :n], t[b, :n]) and 0 <= o[b, n] < V and np.all(o[b, n + 1:] == -1)
+    rows = sorted(np.random.default_rng(2).choice(B, size=64, replace=False).tolist())
+    _check_against_oracle(tgt, drf, toks, ua, us, acc, out, rows=rows)
+
+
+def test_masked_logits_minus_infinity():
+    # logits after top-k style masking: everything outside the top 50 of the TARGET row is -inf in both rows (also whole
+    # 8-element chunks and whole tiles); the kernel must not produce NaN statistics (ADVICE r1)
+    B, gamma, V = 6, 3, 20011
+    lt, ld = I.verify_logits_f32(B, gamma, V, 4242, draft_noise=0.5)
+    for b in range(B):
+        for i in range(gamma + 1):
+            keep = np.argsort(lt[b, i])[-50:]
+            m = np.ones(V, bool)
+            m[keep] = False
+            lt[b, i, m] = -np.inf
+            if i < gamma:
+                ld[b, i, m] = -np.inf
+    toks = I.sample_draft_tokens(_softmax(ld), 4243)
+    acc, out, _ = _run_and_check(lt, ld, toks, I.uniforms((B, gamma), 4244), I.uniforms((B,), 4245), True, torch.float32)
+    assert np.all(out[np.arange(B), acc] >= 0)
+    for b in range(B):
+        assert np.isfinite(lt[b, acc[b], out[b, acc[b]]])        # the drawn token is never a masked one
+
+
 def test_temperature():
     B, gamma, V = 4, 3, 4096
     lt, ld = I.verify_logits_f32(B, gamma, V, 77, draft_noise=0.5)
@@ -145,9 +225,6 @@ def test_every_cluster_size_gives_the_same_tokens(cluster):
     lt, ld = I.verify_logits_f32(B, gamma, V, 911, draft_noise=0.5)
     toks = I.sample_draft_tokens(_softmax(ld), 912)
     ua, us = I.uniforms((B, gamma), 913), I.uniforms((B,), 914)
-    lib = er.load()
-    assert lib.er_verify_tuning(cluster) == 0
-    try:
+    with er.dev_library() as lib:
+        assert lib.er_dev_verify_cluster(cluster) == 0
         _run_and_check(lt, ld, toks, ua, us, True, torch.float32)
-    finally:
-        lib.er_verify_tuning(0)

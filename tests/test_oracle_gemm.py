@@ -97,3 +97,35 @@ def test_bf16_output_rounding_vs_tolerance_finding():
     tol = 1e-2 * np.sqrt(np.mean(y ** 2)) + 1e-3
     y32 = y.astype(np.float32)
     assert np.max(np.abs(y32.astype(np.float64) - y)) < 1e-3 * tol
+
+
+# ---- bf16_gemm (lm_head / target-side linears) ----
+
+def test_bf16_gemm_matches_exact_rational_arithmetic():
+    # pure-Python Fractions on a tiny shape: a transposed operand, a dropped k or a wrong widening fails this
+    from fractions import Fraction
+    rng = np.random.default_rng(5)
+    M, N, K = 3, 4, 7
+    x = O.f32_to_bf16_rne(rng.standard_normal((M, K)).astype(np.float32))
+    w = O.f32_to_bf16_rne((rng.standard_normal((N, K)) * 0.02).astype(np.float32))
+    xf, wf = O.bf16_to_f32(x), O.bf16_to_f32(w)
+    y = O.bf16_gemm(x, w)
+    assert y.shape == (M, N)
+    for m in range(M):
+        for n in range(N):
+            exact = sum(Fraction(float(xf[m, k])) * Fraction(float(wf[n, k])) for k in range(K))
+            assert abs(Fraction(float(y[m, n])) - exact) <= abs(exact) * Fraction(1, 10 ** 12) + Fraction(1, 10 ** 300)
+
+
+def test_bf16_gemm_integers_and_one_hot():
+    rng = np.random.default_rng(6)
+    M, N, K = 5, 6, 256
+    xi = rng.integers(-3, 4, size=(M, K)).astype(np.float32)
+    wi = rng.integers(-8, 8, size=(N, K)).astype(np.float32)
+    y = O.bf16_gemm(O.f32_to_bf16_rne(xi), O.f32_to_bf16_rne(wi))
+    assert np.array_equal(y, (xi.astype(np.int64) @ wi.astype(np.int64).T).astype(np.float64))
+    # one-hot rows read the weight matrix out, transposed
+    eye = np.zeros((K, K), np.float32)
+    eye[np.arange(K), np.arange(K)] = 1
+    w = O.f32_to_bf16_rne(rng.standard_normal((N, K)).astype(np.float32))
+    assert np.array_equal(O.bf16_gemm(O.f32_to_bf16_rne(eye), w), O.bf16_to_f32(w).astype(np.float64).T)
