@@ -61,7 +61,9 @@ __device__ __forceinline__ uint32_t code_bits(float w, float s, float r) {
   return __float_as_uint(t + kMagic);
 }
 __device__ __forceinline__ uint32_t code_bits_div(float w, float s) {  // denormal scales: plain IEEE division
-  return __float_as_uint(__fdiv_rn(w, s) + kMagic);
+  // a bf16 scale below 2^-126 has fewer than 8 significant bits, so amax / s can reach 8 (e.g. amax = 8 ulp, s = 1 ulp):
+  // the clamp of DESIGN.md Q7 is needed here, and only here (rint(clamp(t)) == clamp(rint(t)) for these bounds)
+  return __float_as_uint(fminf(fmaxf(__fdiv_rn(w, s), -8.0f), 7.0f) + kMagic);
 }
 
 // Packs the 8 codes of 4 raw words (k = 0..7 of the word) into one packed word (ER_PACK_V2 keeps this intra-word order): logical k = 2 t + h sits in
