@@ -30,6 +30,7 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 METRIC = "w4a16_drafter_gemm_hbm_gbs_m<=16 (7B layer; +vs-M table, refresh GB/s, verify us in detail)"
+NOMINAL_BF16_TFLOPS = 2250.0
 UNIT = "GB/s"
 NOMINAL_HBM_GBS = 8000.0          # BASELINE.json "~8 TB/s" (context)
 FALLBACK_HBM_GBS = 6650.0         # B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
@@ -37,9 +38,9 @@ W4_BYTES_PER_WEIGHT = 0.5 + 2.0 / 128.0
 REFRESH_BYTES_PER_ELEM = 2.0 + W4_BYTES_PER_WEIGHT
 LAYER_COPIES = 4
 VERIFY_B, VERIFY_GAMMA, VERIFY_V = 64, 4, 152064
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel (w4a16_gemm_kernel<16>,
-# all M<=16 launches of one step) from the ncu --set full capture summarised in profiles/r01_v4_ncu.md.
-NCU_TRAFFIC_BYTES = 30.3e6   # mean over the 20 M<=16 launches of profiles/r01_v4_ncu.md (algorithmic: 30.29e6)
+# roofline.traffic: dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, read at run time from
+# the committed ncu export below (written by the command in profiles/r02_ncu.md); null if the file is missing
+NCU_TRAFFIC_CSV = os.path.join(ROOT, "profiles", "r02_gemm_m_le_16_dram.csv")
 
 
 def log(*a):
@@ -56,6 +57,26 @@ def hbm_peak():
             return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, torch copy)"
     except Exception:
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def bf16_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["bf16_tflops"]), "measured (MEASURED_PEAKS.json bf16_tflops, burst)"
+    except Exception:
+        return 1500.0, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic():
+    """(bytes per launch, source) of the M <= 16 GEMM launches from the committed ncu export, or (None, reason)."""
+    try:
+        import csv
+        with open(NCU_TRAFFIC_CSV) as f:
+            rows = [r for r in csv.DictReader(l for l in f if not l.startswith("#"))]
+        vals = [float(r["dram_read_bytes"]) + float(r["dram_write_bytes"]) for r in rows]
+        return sum(vals) / len(vals), f"profiles/{os.path.basename(NCU_TRAFFIC_CSV)}: mean of {len(vals)} launches"
+    except Exception as e:
+        return None, f"no committed ncu export ({type(e).__name__})"
 
 
 # ------------------------------------------------------------------------------------------------------
@@ -133,8 +154,10 @@ def oracle_threads():
 
 class OracleSample:
     """A bounded sample of the step for the CPU oracle, as it stands (never tuned): refresh of the O
-    projection [3584x3584], its W4A16 linear at M in {1, 16}, and verify of `vb` sequences of the step's
+    projection [3584x3584], its W4A16 linear at M in {1, 16, 256}, and verify of `vb` sequences of the step's
     verify workload (gamma=4, V=152064, bf16 logits).  Inputs are generated once, outside the timing."""
+
+    MS = (1, 16, 256)
 
     def __init__(self, vb=1):
         import numpy as np
@@ -144,14 +167,14 @@ class OracleSample:
         self.N, self.K = 3584, 3584
         self.w = I.as_u16(I.weight_bf16(self.N, self.K, I.seed_of("bench", 0, "o"), device="cpu"))
         self.x = {M: I.as_u16(I.activation_bf16(M, self.K, I.seed_of("bench", "x", M, self.K), device="cpu"))
-                  for M in (1, 16)}
+                  for M in self.MS}
         tgt, drf = I.verify_logits_bf16_device(vb, VERIFY_GAMMA, VERIFY_V, I.seed_of("bench", "verify"), "cpu")
         self.toks = I.sample_draft_tokens_gumbel(drf, I.seed_of("bench", "tok")).numpy()
         self.tgt, self.drf = tgt.float().numpy(), drf.float().numpy()
         self.ua = I.uniforms((vb, VERIFY_GAMMA), 1)
         self.us = I.uniforms((vb,), 2)
         self.vb = vb
-        self.describe = (f"refresh O-proj 3584x3584; W4A16 linear O-proj at M in {{1,16}}; verify {vb} seq "
+        self.describe = (f"refresh O-proj 3584x3584; W4A16 linear O-proj at M in {{1,16,256}}; verify {vb} seq "
                          f"(gamma={VERIFY_GAMMA}, V={VERIFY_V}, bf16 logits)")
 
     def step(self):
@@ -159,7 +182,7 @@ class OracleSample:
         t0 = time.perf_counter()
         qw, sc = O.quantize_pack(self.w)
         t1 = time.perf_counter()
-        for M in (1, 16):
+        for M in self.MS:
             O.w4a16_gemm(self.x[M], qw, sc)
         t2 = time.perf_counter()
         O.spec_verify(self.tgt, self.drf, self.toks, self.ua, self.us, inputs_are_logits=True)
@@ -167,7 +190,7 @@ class OracleSample:
         return t1 - t0, t2 - t1, t3 - t2
 
     def rates(self, tq, tg, tv):
-        gb = sum(gemm_bytes(M, self.N, self.K) for M in (1, 16)) / 1e9
+        gb = sum(gemm_bytes(M, self.N, self.K) for M in self.MS) / 1e9
         return {"gemm_gbs": gb / tg, "refresh_gbs": REFRESH_BYTES_PER_ELEM * self.N * self.K / 1e9 / tq,
                 "verify_us_per_seq": tv / self.vb * 1e6}
 
@@ -220,6 +243,211 @@ def reference_arm(args):
 # ------------------------------------------------------------------------------------------------------
 # product arm
 # ------------------------------------------------------------------------------------------------------
+def _graph_time_us(torch, body, launches, mode, reps=3):
+    """Average microseconds per launch of `body` (which enqueues `launches` kernels on the current stream): captured
+    once in a CUDA graph on a side stream, replayed `reps` + 1 times, best replay, CUDA events on that stream."""
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        if mode == "graph":
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=side):
+                body()
+            run = g.replay
+        else:
+            run = body
+        run()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        best = None
+        for _ in range(reps):
+            e0.record(side)
+            run()
+            e1.record(side)
+            e1.synchronize()
+            t = e0.elapsed_time(e1) * 1e3 / launches
+            best = t if best is None else min(best, t)
+    return best
+
+
+def _random_packed(torch, N, K, dev, gen):
+    """A packed weight matrix with uniformly random nibbles (every nibble is legal input) and scales ~ U(0.001, 0.011):
+    timing passes only need bytes of the right size and layout."""
+    qw = torch.randint(-2 ** 31, 2 ** 31 - 1, (N, K // 8), dtype=torch.int32, device=dev, generator=gen)
+    sc = (torch.rand((K // 128, N), device=dev, generator=gen) * 0.01 + 0.001).to(torch.bfloat16)
+    return qw, sc
+
+
+def gemm_detail(torch, er, I, dev, mode, shape, Ms, peak, l2_bytes, tag):
+    """Per (linear, M): one graph of back-to-back launches rotating through enough DISTINCT weight copies of that one
+    linear that the rotation exceeds 2 x L2 (SURVEY.md 8(d) timing protocol): every row is L2-cold."""
+    gen = torch.Generator(device=dev)
+    gen.manual_seed(I.seed_of("bench", tag))
+    rows = []
+    for name, N, K in shape.linears():
+        wbytes = W4_BYTES_PER_WEIGHT * N * K
+        copies = max(2, int(-(-2.2 * l2_bytes // wbytes)))
+        ws_ = [_random_packed(torch, N, K, dev, gen) for _ in range(copies)]
+        wsb = er.gemm_workspace(max(Ms), N, K, dev)
+        for M in Ms:
+            x = I.activation_bf16(M, K, I.seed_of("bench", "x", M, K), device=dev)
+            y = torch.empty((M, N), dtype=torch.bfloat16, device=dev)
+            R = max(12, copies)
+
+            def body():
+                for r in range(R):
+                    er.w4a16_gemm(x, ws_[r % copies][0], ws_[r % copies][1], y=y, workspace=wsb)
+            us = _graph_time_us(torch, body, R, mode)
+            by = gemm_bytes(M, N, K)
+            rows.append({"linear": name, "N": N, "K": K, "M": M, "us": round(us, 2), "gbs": round(by / us / 1e3, 1),
+                         "frac_of_measured_peak": round(by / us / 1e3 / peak, 4),
+                         "tflops": round(2.0 * M * N * K / us / 1e6, 1), "weight_copies": copies})
+        del ws_
+    return rows
+
+
+def verify_detail(torch, er, I, dev, mode):
+    out = []
+    for B, gamma, V, kind in ((64, 2, 152064, "bf16 logits"), (64, 4, 152064, "bf16 logits"), (64, 8, 152064, "bf16 logits"),
+                              (256, 8, 152064, "bf16 logits"), (4, 4, 32000, "fp32 probs")):
+        if kind == "bf16 logits":
+            tgt, drf = I.verify_logits_bf16_device(B, gamma, V, I.seed_of("bench", "verify", B, gamma), dev)
+            toks = I.sample_draft_tokens_gumbel(drf, I.seed_of("bench", "tok", B, gamma))
+            logits = True
+        else:
+            t32, d32 = I.verify_logits_bf16_device(B, gamma, V, I.seed_of("bench", "verify0"), dev, draft_noise=2.8)
+            toks = I.sample_draft_tokens_gumbel(d32, I.seed_of("bench", "tok0"))
+            tgt, drf = torch.softmax(t32.float(), -1), torch.softmax(d32.float(), -1)   # input generation, not the path
+            logits = False
+        ua = I.uniforms_device((B, gamma), I.seed_of("bench", "ua", B), dev)
+        us_ = I.uniforms_device((B,), I.seed_of("bench", "us", B), dev)
+        acc = torch.empty((B,), dtype=torch.int32, device=dev)
+        o = torch.empty((B, gamma + 1), dtype=torch.int32, device=dev)
+        flush = torch.empty(300 << 20, dtype=torch.uint8, device=dev)
+        R = 4
+
+        def body():
+            for _ in range(R):
+                flush.zero_()                         # the inputs of the small cases fit L2: evict them between launches
+                er.spec_verify(tgt, drf, toks, ua, us_, logits, 1.0, acc, o)
+
+        def body_flush():
+            for _ in range(R):
+                flush.zero_()
+        us = _graph_time_us(torch, body, R, mode) - _graph_time_us(torch, body_flush, R, mode)
+        nbytes = B * (2 * gamma + 1) * V * tgt.element_size()
+        out.append({"B": B, "gamma": gamma, "V": V, "inputs": kind, "us": round(us, 1),
+                    "gbs_if_all_rows_read": round(nbytes / us / 1e3, 1), "mean_accept": round(float(acc.float().mean()), 3)})
+        del tgt, drf, flush
+    return out
+
+
+def model_detail(torch, er, I, dev, mode, peak, gammas=(2, 4, 8), Ms=(256, 128, 64, 16, 4, 1)):
+    """Configs 2 and 3 and SURVEY 8(f) f1 on the whole 7B-shaped model (28 layers, vocab 152064):
+      config 3  refresh of all 112 linears (13.05 GB of bf16 in, 3.365 GB packed out);
+      config 2  the drafter decode step: 28 x (QKV, O, gate/up, down) W4A16 GEMMs chained through real data dependencies
+                (glue stand-ins of SURVEY 8(d): attention := first `hidden` columns of QKV, SiLU(gate) * up, RMS
+                renormalisation -- torch elementwise kernels, timed inside the step and separately) + the bf16 lm_head;
+                per M and gamma: gamma back-to-back steps in ONE CUDA graph + er_spec_verify(B = M, gamma, V);
+      f1        the target model's own step with bf16 weights at M rows (T_p) and at M (gamma + 1) rows (T_V), which
+                turns the above into the paper's Eq. 1  tau * T_p / (gamma * T_q + T_V)."""
+    shape = I.SHAPE_7B
+    lin = shape.linears()
+    H, FF, V, L = shape.hidden, shape.ffn, shape.vocab, shape.layers
+    src = [{n: I.weight_bf16(N, K, I.seed_of("model", l, n), device=dev, outlier_frac=0.001) for n, N, K in lin}
+           for l in range(L)]
+    qw = [{n: torch.empty((N, K // 8), dtype=torch.int32, device=dev) for n, N, K in lin} for _ in range(L)]
+    sc = [{n: torch.empty((K // 128, N), dtype=torch.bfloat16, device=dev) for n, N, K in lin} for _ in range(L)]
+    lm_head = I.weight_bf16(V, H, I.seed_of("model", "lm_head"), device=dev)
+    n_params = sum(N * K for _, N, K in lin) * L
+
+    def refresh_all():
+        for l in range(L):
+            for n, N, K in lin:
+                er.quantize_pack(src[l][n], qw[l][n], sc[l][n])
+    refresh_us = _graph_time_us(torch, refresh_all, 1, mode)
+    refresh = {"linears": L * len(lin), "elements": int(n_params), "ms": round(refresh_us / 1e3, 3),
+               "gbs": round(REFRESH_BYTES_PER_ELEM * n_params / refresh_us / 1e3, 1),
+               "frac_of_measured_peak": round(REFRESH_BYTES_PER_ELEM * n_params / refresh_us / 1e3 / peak, 4),
+               "floor_ms_at_measured_peak": round(REFRESH_BYTES_PER_ELEM * n_params / peak / 1e6, 3)}
+
+    Mmax = max(Ms) * (max(gammas) + 1)
+    ws = torch.empty(max(er.gemm_workspace_bytes(max(Ms), 2 * FF, H), er.load().er_bf16_gemm_workspace_bytes(Mmax, V, H),
+                         er.load().er_bf16_gemm_workspace_bytes(Mmax, 2 * FF, H)), dtype=torch.uint8, device=dev)
+    er._check(er.load().er_gemm_workspace_init(ws.data_ptr(), ws.numel(), torch.cuda.current_stream().cuda_stream), "ws")
+
+    rms = lambda t: torch.nn.functional.rms_norm(t, (t.shape[1],))     # one fused kernel
+
+    def layers(h, linear):
+        # glue stand-ins, as few kernels as possible (they are not on the path): attention := a view of the first `hidden`
+        # columns of QKV (no kernel: the GEMM takes a row stride), residual add + RMS norm, SiLU(gate) * up
+        for l in range(L):
+            qkv = linear(l, "qkv", h)
+            o = linear(l, "o", qkv[:, :H])
+            h2 = rms(h + o)
+            gu = linear(l, "gate_up", h2)
+            d = linear(l, "down", torch.nn.functional.silu(gu[:, :FF]) * gu[:, FF:])
+            h = rms(h2 + d)
+        return h
+
+    def glue_only(h):
+        z = lambda N: torch.zeros((h.shape[0], N), dtype=torch.bfloat16, device=dev)
+        zq, zo, zg, zd = z(lin[0][1]), z(H), z(2 * FF), z(H)
+        return layers(h, lambda l, n, x: {"qkv": zq, "o": zo, "gate_up": zg, "down": zd}[n])
+
+    w4 = lambda l, n, x: er.w4a16_gemm(x, qw[l][n], sc[l][n], workspace=ws)
+    bf = lambda l, n, x: er.bf16_gemm(x, src[l][n], workspace=ws)
+    w4_bytes = W4_BYTES_PER_WEIGHT * n_params
+    lm_bytes = 2.0 * V * H
+    out = {"refresh_whole_model": refresh, "steps": []}
+    for M in Ms:
+        h0 = I.activation_bf16(M, H, I.seed_of("model", "h", M), device=dev)
+        # the parts of one drafter step, each as its own graph
+        t_layers = _graph_time_us(torch, lambda: layers(h0, w4), 1, mode)
+        t_glue = _graph_time_us(torch, lambda: glue_only(h0), 1, mode)
+        t_lm = _graph_time_us(torch, lambda: er.bf16_gemm(h0, lm_head, workspace=ws), 1, mode)
+        t_p = _graph_time_us(torch, lambda: er.bf16_gemm(layers(h0, bf), lm_head, workspace=ws), 1, mode)
+        row = {"M": M, "drafter_w4_layers_us": round(t_layers, 1), "glue_only_us": round(t_glue, 1),
+               "lm_head_bf16_us": round(t_lm, 1),
+               "w4_gbs_excl_glue": round(w4_bytes / max(t_layers - t_glue, 1e-3) / 1e3, 1),
+               "lm_head_gbs": round(lm_bytes / t_lm / 1e3, 1),
+               "T_q_us": round(t_layers + t_lm, 1),
+               "T_q_gbs": round((w4_bytes + lm_bytes) / (t_layers + t_lm) / 1e3, 1),
+               "T_q_floor_us_at_measured_peak": round((w4_bytes + lm_bytes) / peak / 1e3, 1),
+               "T_p_us": round(t_p, 1), "per_gamma": []}
+        for gamma in gammas:
+            tgt, _ = I.verify_logits_bf16_device(M, gamma, V, I.seed_of("model", "tgt", M, gamma), dev)
+            drf = torch.empty((M, gamma, V), dtype=torch.bfloat16, device=dev)
+            toks = torch.randint(0, V, (M, gamma), dtype=torch.int32, device=dev)
+            ua = I.uniforms_device((M, gamma), I.seed_of("model", "ua", M, gamma), dev)
+            us_ = I.uniforms_device((M,), I.seed_of("model", "us", M, gamma), dev)
+            acc = torch.empty((M,), dtype=torch.int32, device=dev)
+            o = torch.empty((M, gamma + 1), dtype=torch.int32, device=dev)
+
+            def sd_iteration():
+                h = h0
+                for i in range(gamma):                      # gamma drafter steps back to back
+                    h = layers(h, w4)
+                    er.bf16_gemm(h, lm_head, y=drf[:, i, :], workspace=ws)
+                    h = rms(drf[:, i, :H])                    # stand-in for the embedding of the drafted token
+                er.spec_verify(tgt, drf, toks, ua, us_, True, 1.0, acc, o)
+            t_sd = _graph_time_us(torch, sd_iteration, 1, mode, reps=2)
+            hv = I.activation_bf16(M * (gamma + 1), H, I.seed_of("model", "hv", M, gamma), device=dev)
+            t_v = _graph_time_us(torch, lambda: er.bf16_gemm(layers(hv, bf), lm_head, workspace=ws), 1, mode, reps=2)
+            t_ver = _graph_time_us(torch, lambda: er.spec_verify(tgt, drf, toks, ua, us_, True, 1.0, acc, o), 1, mode)
+            t_q = t_layers + t_lm
+            row["per_gamma"].append({
+                "gamma": gamma, "drafting_plus_verify_us": round(t_sd, 1), "verify_us": round(t_ver, 1),
+                "T_V_us": round(t_v, 1),
+                # Eq. 1 with the measured times; tau from the paper's own block-efficiency formula at the acceptance the
+                # paper reports for the W4 drafter (alpha = 0.981, PAPER.md:L189) -- the synthetic logits carry no alpha
+                "eq1_speedup_at_alpha_0.981": round(
+                    ((1 - 0.981 ** (gamma + 1)) / (1 - 0.981)) * t_p / (gamma * t_q + t_v + t_ver), 3)})
+            del tgt, drf, hv
+        out["steps"].append(row)
+    del src, qw, sc, lm_head
+    torch.cuda.empty_cache()
+    return out
+
+
 def product_arm(args):
     import torch
     from paper_2606_18967_b200 import er, inputs as I, multi
@@ -363,41 +591,25 @@ def product_arm(args):
             dur[pi, i] = evs[i].elapsed_time(evs[i + 1])
     blk_ms = dur.mean(dim=0)                                   # [refresh, gemm M<=16, gemm M>16, verify]
 
-    # ---- detail pass: every (linear, M) as a graph of R back-to-back launches over the L weight copies ----
-    R = 3 * L
-    det = torch.zeros((len(Ms), len(linears)), dtype=torch.float64)
-    side2 = torch.cuda.Stream()
-    for i, M in enumerate(Ms):
-        for j, (n, N, K) in enumerate(linears):
-            def body():
-                for r in range(R):
-                    er.w4a16_gemm(X[(M, K)], qw[r % L][n], sc[r % L][n], y=Y[n][:M], workspace=ws)
-            with torch.cuda.stream(side2):
-                if mode == "graph":
-                    g = torch.cuda.CUDAGraph()
-                    with torch.cuda.graph(g, stream=side2):
-                        body()
-                    run = g.replay
-                else:
-                    run = body
-                run()
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                best = None
-                for _ in range(3):
-                    e0.record(side2)
-                    run()
-                    e1.record(side2)
-                    e1.synchronize()
-                    t = e0.elapsed_time(e1) / R
-                    best = t if best is None else min(best, t)
-                det[i, j] = best
+    # ---- detail passes (outside the timed step) ------------------------------------------------------------
+    l2_bytes = torch.cuda.get_device_properties(dev).L2_cache_size
+    peak, peak_src = hbm_peak()
+    rows7 = gemm_detail(torch, er, I, dev, mode, I.SHAPE_7B, Ms, peak, l2_bytes, "detail7b")
+    det = torch.tensor([[next(r["us"] for r in rows7 if r["linear"] == n and r["M"] == M) * 1e-3 for n, _, _ in linears]
+                        for M in Ms], dtype=torch.float64)
+    rows32 = verify_rows = model = None
+    if not args.quick:
+        rows32 = gemm_detail(torch, er, I, dev, mode, I.SHAPE_32B, [1, 2, 4, 8, 16, 32], peak, l2_bytes, "detail32b")
+        verify_rows = verify_detail(torch, er, I, dev, mode)
+        del src, qw, sc                      # the whole-model pass needs the memory of the step's layer copies
+        torch.cuda.empty_cache()
+        model = model_detail(torch, er, I, dev, mode, peak)
     torch.cuda.synchronize()
 
     stats = torch.cat([blk_ms, det.flatten(), torch.tensor([step_ms], dtype=torch.float64)])
     stats = multi.max_over_ranks(stats, dist, dev)              # max over ranks, on the device
     blk_ms, det, step_ms = stats[:4], stats[4:-1].reshape(len(Ms), len(linears)), float(stats[-1])
 
-    peak, peak_src = hbm_peak()
     refresh_ms = float(blk_ms[0])
     verify_ms = float(blk_ms[3])
     refresh_bytes = sum(REFRESH_BYTES_PER_ELEM * N * K for _, N, K in linears)
@@ -429,13 +641,14 @@ def product_arm(args):
     # ---- end-to-end leg: the same step through the *_host entry points ---------------------------------
     e2e = None
     if not args.no_e2e:
-        e2e = e2e_leg(args, er, I, torch, dev, linears, Ms, qw, sc, dist, world,
+        e2e = e2e_leg(args, er, I, torch, dev, linears, Ms, dist, world,
                       (v_tgt, v_drf, v_tok, v_ua, v_us), small_bytes)
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         cpu = cpu_baseline_leg()
 
+    traffic, traffic_src = ncu_traffic()
     if rank == 0:
         line = {
             "metric": METRIC, "value": round(value, 1), "unit": UNIT, "n_gpus": world, "steps": args.steps,
@@ -444,22 +657,25 @@ def product_arm(args):
             "config": {"workload": "config1: 7B decoder-layer linear set (QKV 4608x3584, O 3584x3584, gate/up "
                                    "37888x3584, down 3584x18944), W4A16 g128, M in {1..256}; step = refresh of the "
                                    "layer + 36 GEMMs + config-4 verify (B=64, gamma=4, V=152064, bf16 logits)",
-                       "launch": mode, "l2": f"inputs larger than L2: {L} distinct layer copies (470 MB packed) "
+                       "launch": mode, "l2": f"inputs larger than L2: {L} distinct layer copies (480 MB packed) "
                                              "rotated per M; refresh streams 466 MB; verify 175 MB",
                        "per_gpu": "every rank runs the same step on its own sequences/weights (replicas)"},
             "clocks": sampler.summary(),
             "e2e": e2e,
             "gpu_launches": launches_per_step * args.steps,
-            "roofline": {"bound": "hbm", "kernel": "w4a16_gemm_kernel<16, *> (all M<=16 launches of the step; QKV, O, down run the cluster variant)",
+            "roofline": {"bound": "hbm", "kernel": "the 20 er_w4a16_gemm launches at M <= 16 of the step: w4a16_gemm_kernel<16, *> "
+                                                     "(tcgen05; QKV, O, down as clusters) and w4a16_small_kernel<1> (gate/up at M <= 8)",
                          "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
-                         "frac": round(achieved / peak, 4), "traffic": NCU_TRAFFIC_BYTES, "peak_source": peak_src,
+                         "frac": round(achieved / peak, 4), "traffic": traffic, "traffic_source": traffic_src,
+                         "peak_source": peak_src,
                          "bytes_per_launch": round(k16_bytes / k16_n), "us_per_launch": round(k16_ms / k16_n * 1e3, 2)},
             "cpu_baseline": cpu,
             "detail": {
                 "gemm_m_le_16_block_us": round(blk_small_ms * 1e3, 1),
                 "gemm_m_gt_16_block_us": round(float(blk_ms[2]) * 1e3, 1),
-                "gemm_vs_m_method": "detail pass: per (linear, M) one graph of 12 back-to-back launches over the 4 "
-                                    "weight copies, best of 3 replays, per-launch average",
+                "gemm_vs_m_method": "detail pass: per (linear, M) one graph of back-to-back launches rotating through "
+                                    "enough distinct copies of that linear's weights to exceed 2 x L2 (every row is "
+                                    "L2-cold), best of 3 replays, per-launch average",
                 "gemm_vs_m": gemm_table,
                 "refresh": {"us": round(refresh_ms * 1e3, 1), "gbs": round(refresh_bytes / refresh_ms / 1e6, 1),
                             "frac_of_measured_peak": round(refresh_bytes / refresh_ms / 1e6 / peak, 4),
@@ -467,6 +683,9 @@ def product_arm(args):
                 "verify": {"us": round(verify_ms * 1e3, 1), "B": B, "gamma": G, "V": V,
                            "gbs_if_all_rows_read": round(verify_bytes / verify_ms / 1e6, 1),
                            "mean_accept": round(float(v_acc.float().mean()), 3)},
+                "verify_sweep": verify_rows,
+                "config4_32b_gemm_vs_m": rows32,
+                "config2_and_3_whole_model": model,
             },
         }
         print(json.dumps(line), flush=True)
@@ -475,11 +694,16 @@ def product_arm(args):
     return 0
 
 
-def e2e_leg(args, er, I, torch, dev, linears, Ms, qw, sc, dist, world, verify_dev, small_bytes):
+def e2e_leg(args, er, I, torch, dev, linears, Ms, dist, world, verify_dev, small_bytes):
     """The same step with HOST buffers through er_*_host: per step the bf16 weights of the layer, every X and
     the verify inputs are copied host->device from pinned memory and every Y and the verify outputs are read
     back, inside the timed region."""
     L = LAYER_COPIES
+    qw = [{n: torch.empty((N, K // 8), dtype=torch.int32, device=dev) for n, N, K in linears} for _ in range(L)]
+    sc = [{n: torch.empty((K // 128, N), dtype=torch.bfloat16, device=dev) for n, N, K in linears} for _ in range(L)]
+    for c in range(L):
+        for n, N, K in linears:
+            er.quantize_pack(I.weight_bf16(N, K, I.seed_of("bench", c, n), device=dev), qw[c][n], sc[c][n])
     pin = lambda t: t.cpu().pin_memory()
     w_host = {n: pin(I.weight_bf16(N, K, I.seed_of("bench", 0, n), device=dev)) for n, N, K in linears}
     Ks = sorted({K for _, _, K in linears})
@@ -543,6 +767,19 @@ def e2e_leg(args, er, I, torch, dev, linears, Ms, qw, sc, dist, world, verify_de
             "api": "er_quantize_pack_host / er_w4a16_gemm_host / er_spec_verify_host (pinned host buffers)"}
 
 
+def _respawn_under_torchrun(args):
+    """`python bench.py --gpus N` without a torchrun environment: start the N ranks ourselves (one process per GPU,
+    rendezvous on 127.0.0.1) and hand back their exit code; rank 0 of the child job prints the JSON line."""
+    import socket
+    import subprocess
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -552,7 +789,10 @@ def main():
     ap.add_argument("--mode", choices=["graph", "stream"], default="graph")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--quick", action="store_true", help="skip the 32B / verify-sweep / whole-model detail passes")
     args = ap.parse_args()
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        return _respawn_under_torchrun(args)
     if args.impl == "reference":
         return reference_arm(args)
     return product_arm(args)

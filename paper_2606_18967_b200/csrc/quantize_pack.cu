@@ -157,13 +157,6 @@ __device__ __forceinline__ void quantize_tile(const uint16_t* __restrict__ w, in
     const int64_t gg = ((int64_t)bx * kTileK >> 7) + g, n = n0 + r;
     if (n < N && gg < (K >> 7)) scales[gg * N + n] = s_scales[g][r];
   }
-  // The refresh is immediately followed by drafter GEMMs that are launched with programmatic stream serialization and
-  // that start streaming the packed weights BEFORE their griddepcontrol.wait (w4a16_gemm_small.cu).  They may do so
-  // only once every CTA of this kernel has passed this point: the CTA's stores are made visible device-wide (also to
-  // the async proxy the bulk copies read through), then the dependent launch is allowed.
-  __threadfence();
-  asm volatile("fence.proxy.async;" ::: "memory");
-  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 }
 
 __global__ void __launch_bounds__(kThreads) quantize_pack_kernel(const uint16_t* __restrict__ w, int64_t N,

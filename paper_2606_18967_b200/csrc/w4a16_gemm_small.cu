@@ -17,8 +17,10 @@
 //                is handed back as soon as its words sit in registers, at the START of a group's contraction, so the
 //                weight ring is almost entirely bytes in flight.
 //   warp 20      weight producer: one 8 KiB 1-D bulk copy per group (ER_PACK_V2 keeps the block contiguous and
-//                pre-swizzled).  It does not wait for the previous kernel (griddepcontrol.wait): the weights never
-//                depend on it (include/er.h "Ordering").
+//                pre-swizzled).  (Letting it start BEFORE griddepcontrol.wait -- the weights never depend on the
+//                previous GEMM -- was measured and buys nothing: with one CTA per SM this kernel's CTAs only become
+//                resident when the previous kernel's exit; a half-SM variant that does co-reside lost more in the
+//                main loop than it gained.  So the usual stream order holds for every operand.)
 //   warps 21-25  one X warp per worker set: loads the X boxes and the scales of the set's groups and, when they have
 //                landed, sums x[m][k] over the group's 128 k with the tensor cores (A = ones) -- the 136 * sum that
 //                the stored nibble's offset adds to every output of the group (one helper warp for all groups was the
@@ -160,8 +162,8 @@ w4a16_small_kernel(const __grid_constant__ CUtensorMap map_x0, const __grid_cons
   // Programmatic dependent launch: the prologue above touched no global memory and may overlap the tail of the
   // previous kernel in the stream; from here on its results (X, the workspace) are needed.  The next kernel may be
   // scheduled as soon as SMs free up (it waits at its own griddepcontrol.wait).
+  asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-  if (warp != kProdWarp) asm volatile("griddepcontrol.wait;" ::: "memory");   // the weights do not depend on the previous kernel
 
   float tot[2][MB][4];                  // a worker's running sums [row block][n8 block][fragment element]
 

@@ -259,8 +259,8 @@ def test_programmatic_dependent_launch_does_not_change_results():
 
 def test_refresh_then_gemm_back_to_back_sees_the_new_weights():
     # er_quantize_pack immediately followed by er_w4a16_gemm on the same stream, repeatedly with DIFFERENT weights in
-    # the same buffers (the per-RL-step refresh): the GEMM (programmatic dependent launch; the M <= 8
-    # kernel even starts streaming weights before its griddepcontrol.wait) must never read stale packed words
+    # the same buffers (the per-RL-step refresh): the GEMM (programmatic dependent launch: its prologue
+    # overlaps the refresh kernel's tail) must never read stale packed words
     N, K = 37888, 3584
     qw = torch.empty((N, K // 8), dtype=torch.int32, device=DEV)
     sc = torch.empty((K // 128, N), dtype=torch.bfloat16, device=DEV)
