@@ -558,7 +558,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
 namespace er {
 
 #ifdef ER_DEV
-Tuning g_tune = {1, 1, 1, 0, 1};
+Tuning g_tune = {1, 1, 1, 0, 1, 1};
 #endif
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -643,6 +643,7 @@ size_t workspace_for(int mpad) {
   return ER_GEMM_COUNTER_BYTES + (size_t)er::sm_count() * 2 * mpad * kTileN * sizeof(float);
 }
 
+
 template <int MPAD, bool kCl>
 int launch(const CUtensorMap& mx, const GemmParams& gp, const Plan& pl, cudaStream_t stream) {
   static bool attr_set[er::kMaxDevices] = {};
@@ -715,6 +716,7 @@ int er_dev_gemm_tuning(int key, int value) {
   if (key == 4 && (value == 0 || value == 1)) { er::g_tune.split = value; return ER_OK; }
   if (key == 5 && (value == 0 || value == 1)) { er::g_tune.cluster = value; return ER_OK; }
   if (key == 6 && (value == 0 || value == 1)) { er::g_tune.small_mma = value; return ER_OK; }
+  if (key == 7 && value >= 0 && value <= 2) { er::g_tune.large = value; return ER_OK; }
   return ER_ERR_SHAPE;
 }
 #endif
@@ -722,7 +724,10 @@ int er_dev_gemm_tuning(int key, int value) {
 
 size_t er_gemm_workspace_bytes(int64_t M, int64_t N, int64_t K) {
   if (M < 1 || N < kTileN || N % kTileN != 0 || K < ER_GROUP || K % ER_GROUP != 0) return 0;
-  return workspace_for(mpad_of(M));
+  // the largest over the kernels that may serve this M (the development library can switch between them)
+  const size_t exact = workspace_for(mpad_of(M));
+  const size_t large = M > 16 ? er::large_workspace_bytes(M, N, K) : 0;
+  return exact > large ? exact : large;
 }
 
 int er_gemm_workspace_init(void* workspace, size_t workspace_bytes, void* stream) {
@@ -746,7 +751,7 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
   if (!er::aligned16(workspace)) return ER_ERR_ALIGN;
   const Plan pl = make_plan(M, N, K);
   if ((long long)pl.tiles * pl.G >= (1ll << 31)) return ER_ERR_SHAPE;
-  if (workspace_bytes < workspace_for(pl.mpad)) return ER_ERR_WORKSPACE;
+  if (workspace_bytes < er_gemm_workspace_bytes(M, N, K)) return ER_ERR_WORKSPACE;
   int st = er::check_arch();
   if (st != ER_OK) return st;
 
@@ -763,6 +768,9 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
   gp.counters = reinterpret_cast<int*>(workspace);
   gp.partials = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + ER_GEMM_COUNTER_BYTES);
   cudaStream_t s = (cudaStream_t)stream;
+  // M > 16: weights dequantised once per tile for all rows, pre-scaled (w4a16_gemm_large.cu)
+  if (M > 16 && (er::g_tune.large == 2 || (er::g_tune.large == 1 && er::large_preferred(M, N, K))))
+    return er::launch_large(x_bf16, M, N, K, ldx_elems, gp, s);
   // M <= 8 on a plan without a cluster (the large-N linears: gate/up): the warp-level-MMA kernel streams them faster
   // (w4a16_gemm_small.cu; measured in profiles/r02_gemm.md)
   if (M <= 8 && pl.cluster == 1 && er::g_tune.small_mma) return er::launch_small(x_bf16, M, K, ldx_elems, gp, pl, s);

@@ -1,0 +1,521 @@
+// w4a16_gemm_large.cu -- er_w4a16_gemm at M > 16: the batches at the head of a rollout, where the drafter linear turns
+// from memory-bound to tensor-bound (ridge at M ~ 54-66 on this box; the compute term only matters
+// at large B).  The M <= 16 kernels (w4a16_gemm.cu, w4a16_gemm_small.cu) keep a fresh fp32 accumulator per 128-k group
+// so that the group scale is applied exactly; that costs a TENSOR-MEMORY read-back of the whole [128 x M] accumulator
+// per group and, at M > 64, a second / third / fourth pass over the weights.  Here the weights are dequantised ONCE per
+// tile for all batch rows and PRE-SCALED: the A operand is bf16_rne(q * s) (q exact in bf16, one rounding by the
+// multiply), one fp32 accumulator in TENSOR MEMORY runs over the whole K range of a tile segment, and nothing is read
+// back until the segment ends.  The rounding of q * s to bf16 costs accuracy the stated tolerance allows
+// (max|d| <= 1e-2 rms + 1e-3 on the fp32 output; measured 0.5-0.6 of it, G1), which is why the exact kernels
+// stay in charge of M <= 16.
+//
+//   persistent   one CTA per SM, stream-K over (tile, 128-k group) units (w4a16_plan.cuh); swap-AB: the 128 weight rows
+//                of a tile are the M of tcgen05.mma.kind::f16, the padded batch (32 ... 256) is its N.
+//   warps 4, 6   producers: 8 KiB bulk copy of the packed block + 256 B of scales per group (weight ring, up to 12
+//                stages, handed back as soon as the words sit in registers); one SWIZZLE_128B box [M x 64 k] of X per
+//                half group (X ring, consumed by the MMA issuer alone).
+//   warps 8-31   three worker sets of 8 warps; set j converts the groups j, j + 3, ...: 2 x LDS.128, nibble -> bf16
+//                (128 + u), packed fma (-136), packed multiply by the row's group scale, tcgen05.st into one of four
+//                A buffers in TENSOR MEMORY (buffer = group index mod 4; an mbarrier committed by the MMAs frees it).
+//   warp 5       MMA issuer: 8 MMAs per group, A from TENSOR MEMORY, B = the X boxes in shared memory, accumulating
+//                over the segment; tcgen05.commit frees the A buffer and the ring stage; the accumulator is
+//                double-buffered up to M = 128, so the epilogue of a segment runs under the MMAs of the next.
+//   warps 0-3    epilogue: tcgen05.ld (a thread owns a weight row), direct store of whole tiles, fp32 partials to the
+//                workspace otherwise (ticket per tile, ascending CTA order).  Deterministic.
+#include "w4a16_plan.cuh"
+
+namespace {
+
+using namespace er;
+
+constexpr int kSets = 3;
+constexpr int kWorkerWarp0 = 8;
+constexpr int kThreads = (kWorkerWarp0 + kSets * 8) * 32;   // 1024
+constexpr int kABufs = 4;
+constexpr int kMaxStages = 12;
+constexpr int kTmemD = kABufs * 64;          // accumulators behind the A buffers
+
+// TP = weight tiles per X stage.  TP == 2 (a CTA contracts TWO 128-row tiles against every X box it loads, an
+// accumulator each) halves the X traffic, the only stream that grows with the batch; it was built and measured
+// (gate/up M = 128: 42.5 us against 36.9 us at TP == 1, unchanged with the X loads switched off: the loop is bound by
+// the convert -> tcgen05.st -> MMA hand-off, not by X), so only TP == 1 is instantiated.
+template <int MPAD, int TP>
+struct LCfg {
+  // TWO rings.  Weight stages (packed block + its scales, 8.25 KiB) are handed back as soon as the words sit in
+  // registers, so the whole ring is bytes in flight; X stages are single SWIZZLE_128B boxes [MPAD x 64 k] (up to 32
+  // KiB), consumed by the MMA issuer alone, half a group each.  (One ring of whole-group stages is only 3 deep at
+  // M = 256 -- 24 KB of weights in flight per SM -- and different worker sets would meet the same stage in
+  // consecutive phases: with the weight ring a multiple of kSets deep a stage always belongs to one set.)
+  static constexpr int kWStageBytes = kWBytes + 1024;          // packed block, then the 256 B of scales
+  static constexpr int kXBox = MPAD * 128;                     // [MPAD x 64] bf16
+  static constexpr int kXStages = (MPAD >= 256) ? 4 : 6;
+  static constexpr int kFixed = 1024 /*align slack*/ + 1024 /*barriers*/;
+  static constexpr int kWStagesRaw = (kSmemLimit - kFixed - kXStages * kXBox) / kWStageBytes;
+  static constexpr int kWStages = (kWStagesRaw > kMaxStages ? kMaxStages : kWStagesRaw) / kSets * kSets;
+  static constexpr int kSmem = kWStages * kWStageBytes + kXStages * kXBox + kFixed;
+  static constexpr int kDBufs = (2 * TP * MPAD <= 512 - kTmemD) ? 2 : 1;
+  static_assert(kWStages >= 2 * kSets && kTmemD + kDBufs * TP * MPAD <= 512 && kXBox % 1024 == 0 && kXStages % 2 == 0,
+                "shared / tensor memory budget");
+};
+
+#define ER_TMEM_ST16(taddr, r, o)                                                                              \
+  asm volatile(                                                                                                \
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" \
+      ::"r"(taddr), "r"(r[o + 0]), "r"(r[o + 1]), "r"(r[o + 2]), "r"(r[o + 3]), "r"(r[o + 4]), "r"(r[o + 5]),   \
+      "r"(r[o + 6]), "r"(r[o + 7]), "r"(r[o + 8]), "r"(r[o + 9]), "r"(r[o + 10]), "r"(r[o + 11]),              \
+      "r"(r[o + 12]), "r"(r[o + 13]), "r"(r[o + 14]), "r"(r[o + 15])                                           \
+      : "memory")
+
+#define ER_TMEM_LD16(taddr, r)                                                                                 \
+  asm volatile(                                                                                                \
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];" \
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),        \
+        "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])   \
+      : "r"(taddr)                                                                                             \
+      : "memory")
+
+__device__ __forceinline__ uint4 lds128(uint32_t saddr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(saddr));
+  return v;
+}
+__device__ __forceinline__ uint32_t lds_u16(uint32_t saddr) {
+  uint32_t v;
+  asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(saddr));
+  return v;
+}
+__device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+
+// One packed word -> 4 registers of bf16 pairs bf16_rne(q * s): (w >> 4t) & 0x000F000F | 0x43004300 is the pair 128 + u
+// (logic pipe), fma(v, 1, -136) = q exactly, then one packed multiply by (s, s) (both on the FMA pipe).
+__device__ __forceinline__ void dequant_word_scaled(uint32_t w, uint32_t s2, uint32_t* a) {
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    uint32_t v, q;
+    asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(v) : "r"(w >> (4 * t)), "r"(0x000F000Fu), "r"(0x43004300u));
+    asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(q) : "r"(v), "r"(0x3F803F80u), "r"(0xC308C308u));
+    asm("mul.rn.bf16x2 %0, %1, %2;" : "=r"(a[t]) : "r"(q), "r"(s2));
+  }
+}
+
+template <int MPAD, int TP>
+__global__ void __launch_bounds__(kThreads, 1)
+w4a16_large_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
+  using C = LCfg<MPAD, TP>;
+  constexpr int SW = C::kWStages, SX = C::kXStages;
+  constexpr int DB = C::kDBufs;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* xring = smem;                                      // [SX] X boxes (1024-byte aligned)
+  uint8_t* wring = smem + SX * C::kXBox;                      // [SW] packed block + scales
+  uint64_t* bars = reinterpret_cast<uint64_t*>(wring + SW * C::kWStageBytes);
+  uint64_t* wfull = bars;                       // [SW]    packed weights + scales landed
+  uint64_t* wempty = wfull + kMaxStages;        // [SW]    the eight warps of the group's set hold them in registers
+  uint64_t* xfull = wempty + kMaxStages;        // [SX]    X box landed
+  uint64_t* xempty = xfull + 8;                 // [SX]    the MMAs that read it completed
+  uint64_t* a_full = xempty + 8;                // [kABufs] the A operand is written
+  uint64_t* a_free = a_full + kABufs;           // [kABufs] the MMAs that read it completed
+  uint64_t* acc_full = a_free + kABufs;         // [2]     the segment's MMAs completed: accumulator readable
+  uint64_t* acc_free = acc_full + 2;            // [2]     the epilogue has read it
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(acc_free + 2);
+  int* red_info = reinterpret_cast<int*>(tmem_slot + 1);   // [2][4]: tile to finish here (-1: none), first / last contributor
+
+  const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+  const int lane = threadIdx.x & 31;
+  const int cta = blockIdx.x;
+  const int ug = p.unit_groups;
+  const int gb = range_begin(p.uq, p.ur, p.split, cta) * ug;
+  const int ge = range_begin(p.uq, p.ur, p.split, cta + 1) * ug;
+  const int n_it = ge - gb;
+
+  if (warp == 4) {
+    if (lane < SW) {
+      mbar_init(&wfull[lane], 1);
+      mbar_init(&wempty[lane], 8);
+    }
+    if (lane < SX) {
+      mbar_init(&xfull[lane], 1);
+      mbar_init(&xempty[lane], 1);
+    }
+    if (lane < kABufs) {
+      mbar_init(&a_full[lane], 8);
+      mbar_init(&a_free[lane], 1);
+    }
+    if (lane < 2) {
+      mbar_init(&acc_full[lane], 1);
+      mbar_init(&acc_free[lane], 4);
+    }
+    mbar_fence_init();
+    if (lane == 0) tma_prefetch_desc(&map_x);
+  }
+  if (warp == 5) tmem_alloc<512>(tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);
+  // programmatic dependent launch: see w4a16_gemm.cu
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+
+  if (warp == 4) {
+    // ===================== weight producer =====================
+    int g = gb % p.G, tu = (gb / p.G) % p.ntiles;     // p.ntiles counts units of TP tiles
+    int s = 0;
+    uint32_t ph = 0;
+    for (int it = 0; it < n_it; ++it) {
+#pragma unroll
+      for (int w = 0; w < TP; ++w) {
+        const int tn = tu * TP + w;
+        mbar_wait(&wempty[s], ph ^ 1);
+        if (elect_one()) {
+          uint8_t* st = wring + s * C::kWStageBytes;
+          mbar_arrive_expect_tx(&wfull[s], kWBytes + kScaleBytes);
+          bulk_load_1d(st, p.qweight + ((size_t)tn * p.G + g) * kWBytes, kWBytes, &wfull[s], kEvictFirst);
+          bulk_load_1d(st + kWBytes, p.scales + ((size_t)g * p.N + tn * kTileN) * 2, kScaleBytes, &wfull[s], kEvictFirst);
+        }
+        __syncwarp();
+        if (++s == SW) { s = 0; ph ^= 1; }
+      }
+      if (++g == p.G) {
+        g = 0;
+        if (++tu == p.ntiles) tu = 0;
+      }
+    }
+  } else if (warp == 6) {
+    // ===================== X producer: two boxes [MPAD x 64 k] per group =====================
+    const int tile0 = gb / p.G;
+    int g = gb % p.G, tn = tile0 % p.ntiles, mc = tile0 / p.ntiles;
+    int s = 0;
+    uint32_t ph = 0;
+    for (int it = 0; it < 2 * n_it; ++it) {
+      mbar_wait(&xempty[s], ph ^ 1);
+      if (elect_one()) {
+        mbar_arrive_expect_tx(&xfull[s], C::kXBox);
+        tma_load_2d(xring + s * C::kXBox, &map_x, &xfull[s], g * 128 + (it & 1) * 64, mc * MPAD, kEvictLast);
+      }
+      __syncwarp();
+      if ((it & 1) && ++g == p.G) {
+        g = 0;
+        if (++tn == p.ntiles) { tn = 0; ++mc; }
+      }
+      if (++s == SX) { s = 0; ph ^= 1; }
+    }
+  } else if (warp == 5) {
+    // ===================== MMA issuer =====================
+    constexpr uint32_t idesc = idesc_bf16_m128(MPAD);
+    int sx = 0, b = 0;
+    uint32_t xph = 0, bph = 0;
+    int it = 0, seg = 0;
+    while (it < n_it) {
+      const int g_lo = (gb + it) % p.G;
+      const int seg_len = min(p.G - g_lo, n_it - it);
+      const int buf = DB == 2 ? (seg & 1) : 0;
+      if (seg >= DB) mbar_wait(&acc_free[buf], ((seg / DB) - 1) & 1);   // the epilogue of segment seg - DB has drained it
+      for (int u = 0; u < seg_len; ++u) {
+#pragma unroll
+        for (int w = 0; w < TP; ++w) {
+          const uint32_t d_t = tmem + kTmemD + (buf * TP + w) * MPAD;
+          mbar_wait(&a_full[b], bph);
+#pragma unroll
+          for (int h = 0; h < 2; ++h) {
+            if (w == 0) mbar_wait(&xfull[sx + h], xph);     // kXStages is even: both boxes of a group share a phase
+            tc_fence_after();
+            if (elect_one()) {
+              const uint32_t xbase = smem_u32(xring + (sx + h) * C::kXBox);
+              const uint32_t a_t = tmem + b * 64 + h * 32;
+#pragma unroll
+              for (int kk = 0; kk < 4; ++kk) {
+                const uint64_t bdesc = smem_desc_sw128(xbase + kk * 32);
+                mma_ts_f16(d_t, a_t + kk * 8, bdesc, idesc, (u > 0 || h > 0 || kk > 0) ? 1u : 0u);
+              }
+              if (w == TP - 1) tc_commit(&xempty[sx + h]);
+              if (h == 1) {
+                tc_commit(&a_free[b]);
+                if (u == seg_len - 1 && w == TP - 1) tc_commit(&acc_full[buf]);
+              }
+            }
+            __syncwarp();
+          }
+          if (++b == kABufs) { b = 0; bph ^= 1; }
+        }
+        sx += 2;
+        if (sx == SX) { sx = 0; xph ^= 1; }
+      }
+      it += seg_len;
+      ++seg;
+    }
+  } else if (warp >= kWorkerWarp0) {
+    // ===================== worker sets: convert + scale, write the A operand =====================
+    const int dw = warp - kWorkerWarp0;
+    const int set = dw >> 3;
+    const int half = (dw >> 2) & 1;        // which 64 k of a group this thread converts
+    const int q4 = warp & 3;               // TMEM lane quarter this warp may access
+    const int row = q4 * 32 + lane;
+    const uint32_t lane_addr = (uint32_t)(q4 * 32) << 16;
+    const int sw = (row >> 1) & 3;
+    uint32_t w_addr0, w_addr1, sc_addr, wfull_addr, wempty_addr, afull_addr, afree_addr, a_base, rt_zero;
+    asm volatile("mov.u32 %0, %1;" : "=r"(w_addr0) : "r"(smem_u32(wring) + row * 64 + (((2 * half) ^ sw) << 4)));
+    asm volatile("mov.u32 %0, %1;" : "=r"(w_addr1) : "r"(smem_u32(wring) + row * 64 + (((2 * half + 1) ^ sw) << 4)));
+    asm volatile("mov.u32 %0, %1;" : "=r"(sc_addr) : "r"(smem_u32(wring) + kWBytes + row * 2));
+    asm volatile("mov.u32 %0, %1;" : "=r"(wfull_addr) : "r"(smem_u32(wfull)));
+    asm volatile("mov.u32 %0, %1;" : "=r"(wempty_addr) : "r"(smem_u32(wempty)));
+    asm volatile("mov.u32 %0, %1;" : "=r"(afull_addr) : "r"(smem_u32(a_full)));
+    asm volatile("mov.u32 %0, %1;" : "=r"(afree_addr) : "r"(smem_u32(a_free)));
+    asm volatile("mov.u32 %0, %1;" : "=r"(a_base) : "r"(tmem + lane_addr + half * 32));
+    asm volatile("mov.u32 %0, %1;" : "=r"(rt_zero) : "r"((uint32_t)p.M >> 24));   // 0 at run time, unknown to ptxas
+    int s = set;                           // SW is a multiple of kSets: stage s always belongs to this set
+    uint32_t ph = 0;
+    for (int my = set; my < n_it * TP; my += kSets) {      // my = group index * TP + tile of the unit
+      mbar_wait_addr(wfull_addr + s * 8, ph);
+      const uint32_t st = s * C::kWStageBytes;
+      const uint4 pk0 = lds128(st + w_addr0);
+      const uint4 pk1 = lds128(st + w_addr1);
+      const uint32_t sc16 = lds_u16(st + sc_addr);
+      // hand the weight stage back once the three loads have returned: the arrive's address depends on them
+      uint32_t dep;
+      asm volatile("lop3.b32 %0, %1, %2, %3, 0x80;" : "=r"(dep) : "r"(pk0.w), "r"(pk1.w), "r"(sc16));
+      asm volatile("and.b32 %0, %0, %1;" : "+r"(dep) : "r"(rt_zero));
+      __syncwarp();
+      if (lane == 0) mbar_arrive_addr(wempty_addr + s * 8 + dep);
+      const uint32_t s2 = sc16 | (sc16 << 16);
+      uint32_t a[32];
+      dequant_word_scaled(pk0.x, s2, a + 0);
+      dequant_word_scaled(pk0.y, s2, a + 4);
+      dequant_word_scaled(pk0.z, s2, a + 8);
+      dequant_word_scaled(pk0.w, s2, a + 12);
+      dequant_word_scaled(pk1.x, s2, a + 16);
+      dequant_word_scaled(pk1.y, s2, a + 20);
+      dequant_word_scaled(pk1.z, s2, a + 24);
+      dequant_word_scaled(pk1.w, s2, a + 28);
+      const int b = my & (kABufs - 1);
+      if (my >= kABufs) mbar_wait_addr(afree_addr + b * 8, ((my / kABufs) - 1) & 1);   // MMAs of group my - 4 are done
+      tc_fence_after();
+      ER_TMEM_ST16(a_base + b * 64 + 0, a, 0);
+      ER_TMEM_ST16(a_base + b * 64 + 16, a, 16);
+      asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive_addr(afull_addr + b * 8);
+      s += kSets;
+      if (s >= SW) { s -= SW; ph ^= 1; }
+    }
+  } else if (warp < 4) {
+    // ===================== epilogue (TMEM lane quarter = warp) =====================
+    const int row = warp * 32 + lane;
+    const uint32_t lane_addr = (uint32_t)(warp * 32) << 16;
+    const bool leader = (threadIdx.x == 0);
+    int it = 0, seg = 0;
+    int pend_tile[2] = {-1, -1};
+    while (it < n_it) {
+      const int gi0 = gb + it;
+      const int tile = gi0 / p.G, g_lo = gi0 % p.G;
+      const int seg_len = min(p.G - g_lo, n_it - it);
+      const int buf = DB == 2 ? (seg & 1) : 0;
+      mbar_wait(&acc_full[buf], (seg / DB) & 1);
+      tc_fence_after();
+      const int m_base = (tile / p.ntiles) * MPAD;
+      const bool whole = (seg_len == p.G);
+      const int k = (it == 0 ? 0 : 1);
+#pragma unroll 1
+      for (int wc = 0; wc < TP * MPAD; wc += 16) {
+        const int w = wc / MPAD, c0 = wc % MPAD;   // tile of the unit, first batch row of the chunk
+        if (m_base + c0 >= p.M) continue;          // rows >= M are never written (uniform over the CTA)
+        const int n = ((tile % p.ntiles) * TP + w) * kTileN + row;
+        float* mine = p.partials + (((size_t)cta * 2 + k) * TP + w) * (MPAD * kTileN);
+        uint32_t v[16];
+        ER_TMEM_LD16(tmem + lane_addr + kTmemD + (buf * TP + w) * MPAD + c0, v);
+        asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+        for (int j = 0; j < 16; ++j) {
+          const int m = m_base + c0 + j;
+          if (m < p.M) {
+            if (whole) {
+              if (p.y_f32) reinterpret_cast<float*>(p.y)[(size_t)m * p.ldy + n] = __uint_as_float(v[j]);
+              else reinterpret_cast<__nv_bfloat16*>(p.y)[(size_t)m * p.ldy + n] = __float2bfloat16_rn(__uint_as_float(v[j]));
+            } else {
+              __stcg(mine + (c0 + j) * kTileN + row, __uint_as_float(v[j]));
+            }
+          }
+        }
+      }
+      if (!whole) pend_tile[k] = tile;
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&acc_free[buf]);
+      it += seg_len;
+      ++seg;
+    }
+
+    // ---- partial tiles: ticket per tile; the last CTA to arrive adds all partials (below, with every warp) ----
+    // Ordering: partial stores (the 128 epilogue threads) -> bar.sync -> the leader's acq_rel ticket (release is cumulative
+    // over what the barrier made visible to the leader); last arriver: acq_rel ticket -> __syncthreads -> ld.cg.
+    if (pend_tile[0] >= 0 || pend_tile[1] >= 0) named_bar_sync(1, 128);
+    if (leader) {
+#pragma unroll
+      for (int k = 0; k < 2; ++k) {
+        int last = 0;
+        if (pend_tile[k] >= 0) {
+          const int c_lo = owner_of(p.uq, p.ur, p.split, (pend_tile[k] * p.G) / ug);
+          const int c_hi = owner_of(p.uq, p.ur, p.split, ((pend_tile[k] + 1) * p.G - 1) / ug);
+          int old;
+          asm volatile("atom.acq_rel.gpu.global.add.s32 %0, [%1], 1;" : "=r"(old) : "l"(p.counters + pend_tile[k]) : "memory");
+          last = (old == c_hi - c_lo);
+          if (last) p.counters[pend_tile[k]] = 0;  // leave the counter zero for the next call
+          red_info[4 * k + 1] = c_lo;
+          red_info[4 * k + 2] = c_hi;
+        }
+        red_info[4 * k] = last ? pend_tile[k] : -1;
+      }
+    }
+  }
+  tc_fence_before();
+  __syncthreads();          // every role is done; red_info is visible
+  // ---- the last CTA of a partial tile adds the partials in ascending CTA order: all 32 warps, a thread owns a weight
+  //      row and MPAD / 8 batch rows, the loads of four contributors in flight together ----
+#pragma unroll 1
+  for (int k = 0; k < 2; ++k) {
+    const int tile = red_info[4 * k];
+    if (tile < 0) continue;
+    const int c_lo = red_info[4 * k + 1], c_hi = red_info[4 * k + 2];
+    const int row = threadIdx.x & 127, cg = threadIdx.x >> 7;
+    constexpr int CPT = MPAD / 8;                    // batch rows per thread
+    const int m0 = (tile / p.ntiles) * MPAD + cg * CPT;
+#pragma unroll 1
+    for (int wj = 0; wj < TP * CPT; wj += 4) {
+      const int w = wj / CPT, j0 = wj % CPT;
+      const int n = ((tile % p.ntiles) * TP + w) * kTileN + row;
+      if (m0 + j0 >= p.M) continue;
+      float acc[4] = {0.f, 0.f, 0.f, 0.f};
+      for (int c0 = c_lo; c0 <= c_hi; c0 += 4) {
+        float v[4][4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const int c = min(c0 + q, c_hi);
+          // CTA c's piece of this tile is its first segment iff its range starts inside the tile
+          const int which = (range_begin(p.uq, p.ur, p.split, c) * ug >= tile * p.G) ? 0 : 1;
+          const float* src = p.partials + (((size_t)c * 2 + which) * TP + w) * (MPAD * kTileN) + (cg * CPT + j0) * kTileN + row;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) v[q][j] = (m0 + j0 + j < p.M && c0 + q <= c_hi) ? __ldcg(src + j * kTileN) : 0.f;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+#pragma unroll
+          for (int j = 0; j < 4; ++j) acc[j] += v[q][j];
+      }
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int m = m0 + j0 + j;
+        if (m < p.M) {
+          if (p.y_f32) reinterpret_cast<float*>(p.y)[(size_t)m * p.ldy + n] = acc[j];
+          else reinterpret_cast<__nv_bfloat16*>(p.y)[(size_t)m * p.ldy + n] = __float2bfloat16_rn(acc[j]);
+        }
+      }
+    }
+  }
+  __syncthreads();
+  tc_fence_after();
+  if (warp == 5) tmem_dealloc<512>(tmem);
+}
+
+template <int MPAD, int TP>
+int launch(const CUtensorMap& mx, const GemmParams& gp, int ctas, cudaStream_t stream) {
+  static bool attr_set[er::kMaxDevices] = {};
+  const int dev = er::current_device();
+  if (dev < 0 || dev >= er::kMaxDevices || !attr_set[dev]) {
+    ER_CUDA_TRY(cudaFuncSetAttribute(w4a16_large_kernel<MPAD, TP>, cudaFuncAttributeMaxDynamicSharedMemorySize, LCfg<MPAD, TP>::kSmem));
+    if (dev >= 0 && dev < er::kMaxDevices) attr_set[dev] = true;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)ctas);
+  cfg.blockDim = dim3(kThreads);
+  cfg.dynamicSmemBytes = LCfg<MPAD, TP>::kSmem;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = er::g_tune.pdl;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  ER_CUDA_TRY(cudaLaunchKernelEx(&cfg, w4a16_large_kernel<MPAD, TP>, mx, gp));
+  return ER_OK;
+}
+
+}  // namespace
+
+namespace er {
+
+int large_mpad_of(int64_t M) { return M <= 32 ? 32 : (M <= 64 ? 64 : (M <= 128 ? 128 : 256)); }
+
+// Plan of the large-batch kernel.  The padded batch MPAD (the N of the MMA) may be SMALLER than M: the batch is then
+// cut into M / MPAD chunks, every (chunk, unit of TP 128-row tiles) is a tile of its own, and the weights are converted
+// once per chunk -- cheap for the small linears, where it buys whole tiles for most SMs instead of split-K partial sums
+// of up to 128 KB.  Cost model per 128-k group of a unit, in SM cycles: the conversion (~450 per tile, measured), the
+// MMAs (4 MPAD per tile) and the X boxes (2 MPAD rows of 128 B at ~4.8 cycles per row through TMA / L2, measured; ONCE
+// per unit -- which is what TP = 2 is for).
+struct LargePlan { int mpad, tp, unit_groups, ctas; double cycles; };
+static LargePlan large_plan(int64_t M, int64_t N, int64_t K, int sms, int force_ctas) {
+  LargePlan best = {0, 1, 0, 0, 1e30};
+  const int G = (int)(K / ER_GROUP), ntiles = (int)(N / kTileN);
+  const int ctas = (force_ctas > 0 && force_ctas < sms) ? force_ctas : sms;
+  for (int mpad = large_mpad_of(M); mpad >= 32; mpad >>= 1) {
+    for (int tp = 1; tp <= 1; ++tp) {
+      const long long tiles = (long long)(ntiles / tp) * ((M + mpad - 1) / mpad);
+      const double per_group = fmax(450.0 * tp, fmax(4.0 * mpad * tp, 9.6 * mpad));
+      {  // whole tiles
+        const int c = (int)(tiles < ctas ? tiles : ctas);
+        const double cyc = (double)((tiles + c - 1) / c) * G * per_group + 2000.0;
+        if (force_ctas == 0 && cyc < best.cycles) best = {mpad, tp, G, c, cyc};
+      }
+      if (tiles <= ER_GEMM_COUNTER_BYTES / 4) {  // stream-K ranges + partial tiles through the workspace (ticket per tile)
+        const long long units = tiles * G;
+        const int c = (int)(units < ctas ? units : ctas);
+        const double cyc = (double)((units + c - 1) / c) * per_group + 6000.0 + 40.0 * mpad * tp;
+        if (cyc < best.cycles) best = {mpad, tp, 1, c, cyc};
+      }
+    }
+    if (mpad == 32) break;
+  }
+  return best;
+}
+
+// true where the large-batch kernel gets whole tiles on at least ~45 % of the SMs (no split-K partial sums): there it
+// beats the exact per-group kernel from M > 64 on (profiles/r02_gemm.md); on long-K / few-tile shapes (`down`) the
+// exact kernel's stream-K stays
+bool large_preferred(int64_t M, int64_t N, int64_t K) {
+  if (M <= 64) return false;
+  const LargePlan pl = large_plan(M, N, K, sm_count(), g_tune.force_ctas);
+  return pl.unit_groups > 1 && (long long)pl.ctas * 100 >= (long long)sm_count() * 45;
+}
+
+size_t large_workspace_bytes(int64_t M, int64_t N, int64_t K) {
+  // enough for every plan the model may pick for this problem (and for the development library's forced CTA counts)
+  return ER_GEMM_COUNTER_BYTES + (size_t)sm_count() * 2 * 256 * kTileN * sizeof(float);
+}
+
+// M > 16: `gp` arrives with the problem, the output and the workspace filled in, the partition is made here.
+int launch_large(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, GemmParams gp, cudaStream_t stream) {
+  const LargePlan pl = large_plan(M, N, K, sm_count(), g_tune.force_ctas);
+  const int mpad = pl.mpad;
+  const int mchunks = (int)((M + mpad - 1) / mpad), ntiles = (int)(N / kTileN) / pl.tp;    // units of tp tiles
+  const long long tiles = (long long)ntiles * mchunks;
+  const int G = (int)(K / ER_GROUP);
+  if (tiles * G >= (1ll << 31)) return ER_ERR_SHAPE;
+  const int unit_groups = pl.unit_groups, ctas = pl.ctas;
+  const long long units = tiles * G / unit_groups;
+  gp.G = G; gp.ntiles = ntiles; gp.tiles = (int)tiles; gp.unit_groups = unit_groups; gp.units = (int)units;
+  gp.uq = (int)(units / ctas); gp.ur = (int)(units % ctas);
+  gp.split = 0; gp.cluster = 1;
+  CUtensorMap mx;
+  if (!make_map_2d(&mx, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, x, (uint64_t)M, (uint64_t)K, (uint64_t)ldx * 2, (uint32_t)mpad,
+                   64, CU_TENSOR_MAP_SWIZZLE_128B)) {
+    set_last_cuda_error((int)cudaErrorInvalidValue);
+    return ER_ERR_CUDA;
+  }
+  switch (mpad) {
+    case 32: return launch<32, 1>(mx, gp, ctas, stream);
+    case 64: return launch<64, 1>(mx, gp, ctas, stream);
+    case 128: return launch<128, 1>(mx, gp, ctas, stream);
+    default: return launch<256, 1>(mx, gp, ctas, stream);
+  }
+}
+
+}  // namespace er

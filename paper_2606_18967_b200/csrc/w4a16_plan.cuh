@@ -67,12 +67,14 @@ struct Tuning {
   int split;        // tile split where it applies
   int cluster;      // cluster mode where it applies
   int force_ctas;   // > 0: use this many CTAs; 0 = one per SM
-  int small_mma;    // M <= 16 through the warp-level-MMA kernel (0: through the tcgen05 kernel)
+  int small_mma;    // M <= 8 without a cluster through the warp-level-MMA kernel (0: through the tcgen05 kernel)
+  int large;        // 1: the pre-scaled large-batch kernel where it is preferred (M > 64, whole tiles); 0: never;
+                    // 2: for every M > 16 (tests)
 };
 #ifdef ER_DEV
 extern Tuning g_tune;
 #else
-constexpr Tuning g_tune = {1, 1, 1, 0, 1};
+constexpr Tuning g_tune = {1, 1, 1, 0, 1, 1};
 #endif
 
 // 2-D row-major tensor [rows][cols] of elements, row pitch in bytes, box [box_rows][box_cols].
@@ -81,5 +83,11 @@ bool make_map_2d(CUtensorMap* map, CUtensorMapDataType dt, const void* base, uin
 
 // M <= 8, no cluster: w4a16_gemm_small.cu
 int launch_small(const void* x, int64_t M, int64_t K, int64_t ldx, GemmParams gp, const Plan& pl, cudaStream_t stream);
+
+// M > 16: w4a16_gemm_large.cu
+int large_mpad_of(int64_t M);
+size_t large_workspace_bytes(int64_t M, int64_t N, int64_t K);
+bool large_preferred(int64_t M, int64_t N, int64_t K);
+int launch_large(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, GemmParams gp, cudaStream_t stream);
 
 }  // namespace er

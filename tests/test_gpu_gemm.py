@@ -166,7 +166,10 @@ def _sampled_columns_check(x, qw, sc, N, K, seed, label, y=None):
     assert err_s <= _tol(y_ref), f"{label} M={M}: SIMT max|d|={err_s}"
     rms = float(y_simt.float().pow(2).mean().sqrt())
     gap = float((y - y_simt).abs().max())
-    assert gap <= 1e-4 * rms + 1e-5, f"{label} M={M}: tcgen05 vs SIMT over all columns: {gap} (rms {rms})"
+    # (M > 64 may be served by the large-batch kernel, whose A operand is bf16_rne(q * s): there the gap to the exact
+    # CUDA-core result is the rounding the stated tolerance allows, not a summation-order effect)
+    gap_tol = 1e-4 * rms + 1e-5 if M <= 64 else 1e-2 * rms + 1e-3
+    assert gap <= gap_tol, f"{label} M={M}: tensor-core kernel vs SIMT over all columns: {gap} (rms {rms})"
     assert torch.isfinite(y).all()
     return y
 
@@ -331,3 +334,56 @@ def test_heavy_tailed_activations_stay_within_tolerance(M):
     mask = torch.rand(M, K, generator=g) < 0.002
     x = torch.where(mask, x * 100.0, x).to(torch.bfloat16).to(DEV)
     _check(x, qw, sc)
+
+
+@pytest.mark.parametrize("M", [17, 32, 33, 64, 100, 128, 129, 256, 300])
+def test_large_batch_kernel_every_m(M):
+    # w4a16_gemm_large.cu (A operand = bf16_rne(q * s), one accumulator over K) forced for every M > 16 through the
+    # development library: whole tiles, stream-K ranges with partial tiles (forced CTA counts), several batch chunks
+    # (M = 300 > 256), ragged M; within the stated tolerance of the oracle and bit-identical run to run
+    N, K = 1024, 1152
+    w = I.weight_bf16(N, K, I.seed_of("large", "w"), device=DEV)
+    x = I.activation_bf16(M, K, I.seed_of("large", "x", M), device=DEV)
+    qw, sc = er.quantize_pack(w)
+    y_ref = O.w4a16_gemm(I.as_u16(x), qw.cpu().numpy().view(np.uint32), I.as_u16(sc))
+    with er.dev_library() as lib:
+        assert lib.er_dev_gemm_tuning(7, 2) == 0
+        for ctas in (0, 5, 37):
+            assert lib.er_dev_gemm_tuning(1, ctas) == 0
+            y1 = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
+            y2 = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
+            yb = er.w4a16_gemm(x, qw, sc, out_dtype=torch.bfloat16)
+            torch.cuda.synchronize()
+            err = np.abs(y1.cpu().numpy().astype(np.float64) - y_ref).max()
+            assert err <= _tol(y_ref), (M, ctas, err, _tol(y_ref))
+            assert torch.equal(y1, y2)
+            assert np.array_equal(I.as_u16(yb), O.f32_to_bf16_rne(y1.cpu().numpy()))
+
+
+def test_large_batch_kernel_exact_cases():
+    # power-of-two scales: q * s is exact in bf16, so the large-batch kernel must reproduce the integer probe bit for bit
+    # (pins its layout, k order, accumulate flags and split-K reduction); general scales: a one-hot X reads out
+    # bf16_rne(q * s) exactly
+    N, K, M = 256, 3584, 200
+    codes = I.random_codes(N, K, 21)
+    su = np.full((K // 128, N), 0x3F80, dtype=np.uint16)
+    su[1::2] = 0x4000
+    qw, sc = _dev_weights(codes, su)
+    rng = np.random.default_rng(3)
+    x = torch.from_numpy(rng.integers(-1, 3, size=(M, K)).astype(np.float32)).to(DEV).to(torch.bfloat16)
+    ref = O.w4a16_gemm(I.as_u16(x), qw.cpu().numpy().view(np.uint32), su)
+    su2 = _random_scales(K // 128, N, 22)
+    qw2, sc2 = _dev_weights(codes, su2)
+    wd = O.dequantize(O.pack_codes(codes), su2)                   # fp64 q * s
+    wd_bf16 = O.bf16_to_f32(O.f32_to_bf16_rne(wd.astype(np.float32))).astype(np.float64)
+    with er.dev_library() as lib:
+        lib.er_dev_gemm_tuning(7, 2)
+        for ctas in (0, 11):
+            lib.er_dev_gemm_tuning(1, ctas)
+            y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
+            assert np.array_equal(y.cpu().numpy().astype(np.float64), ref), ctas
+        lib.er_dev_gemm_tuning(1, 0)
+        xo = torch.zeros((256, K), dtype=torch.bfloat16, device=DEV)
+        xo[torch.arange(256), 1000 + torch.arange(256)] = 1.0
+        y = er.w4a16_gemm(xo, qw2, sc2, out_dtype=torch.float32).cpu().numpy().astype(np.float64)
+        assert np.array_equal(y, wd_bf16[:, 1000:1256].T)
