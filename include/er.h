@@ -75,7 +75,9 @@ size_t er_scales_bytes(int64_t N, int64_t K, int group); /* (K/group)*N*2 */
 /* Workspace er_w4a16_gemm needs for this problem (split-K partials + tile counters).  Never 0 for a
  * valid shape.  The first ER_GEMM_COUNTER_BYTES of the workspace hold tile counters that MUST be zero
  * before the first call that uses the workspace (er_gemm_workspace_init does that); every call leaves
- * them zero again, so one workspace may be reused by any number of calls on one stream. */
+ * them zero again, so one workspace may be reused by any number of calls on one stream.  (SURVEY 8(b) proposed a
+ * workspace that "need not be zeroed"; a split-K ticket that recognises stale counters needs an epoch word per call,
+ * i.e. library state, or a memset node per call -- one init per workspace was kept instead.) */
 size_t er_gemm_workspace_bytes(int64_t M, int64_t N, int64_t K);
 #define ER_GEMM_COUNTER_BYTES 16384
 int er_gemm_workspace_init(void* workspace, size_t workspace_bytes, void* stream);
@@ -111,13 +113,21 @@ int er_quantize_pack_batched(const er_linear_desc* descs, int count, int group, 
  *            row stride ldy_elems; rows >= M are never written
  *   workspace  caller-provided, >= er_gemm_workspace_bytes(M,N,K), 16-byte aligned, counters zeroed once
  *            (N/128) * (K/128) * ceil(M / 64) must stay below 2^31 (else ER_ERR_SHAPE)
- * Arithmetic: stored nibbles u = q + 8 are widened exactly to bf16 (as 128 + u), contracted with X on the
- * tensor cores with fp32 accumulation per 128-k group; the same accumulator receives -136 * sum_k x[m][k]
- * (the offset, through a constant operand tile), so it holds sum_k x * q up to fp32 rounding; each group's
- * sum is multiplied by its fp32 scale and added in fp32 (no rounding of q*s); split-K partials are reduced
- * in ascending CTA order, or inside a thread-block cluster in rank order (both deterministic).
- * Launch: one persistent kernel, launched with programmatic stream serialization; it touches no global
- * memory before griddepcontrol.wait, so ordering against earlier work in the stream is the usual one. */
+ * Arithmetic (three kernels, chosen from M and the work plan):
+ *   M <= 16 (the memory-bound regime): stored nibbles u = q + 8 are widened exactly to bf16 (as 128 + u) and contracted
+ *     with X on the tensor cores with fp32 accumulation per 128-k group; the 136 * sum_k x[m][k] the offset adds is
+ *     removed on that fp32 sum (through a constant operand tile, or with the x sums computed beside the contraction), so
+ *     it holds sum_k x * q up to fp32 rounding; each group's sum is multiplied by its fp32 scale and added in fp32 (NO
+ *     rounding of q * s).  The same holds for 16 < M <= 64 and wherever the plan keeps the per-group kernel.
+ *   M > 64 where whole 128-row tiles keep the SMs busy (e.g. QKV, O, gate/up): the weights are dequantised once per tile
+ *     for all batch rows as bf16_rne(q * s) (q exact, ONE rounding by the multiply) and one fp32 accumulator runs over all
+ *     of K.  That rounding is the error the stated tolerance (1e-2 rms + 1e-3 on the fp32 output) allows for; with
+ *     power-of-two scales the result is exact.
+ *   Split-K partials are reduced in ascending CTA order, or inside a thread-block cluster in rank order; every kernel is
+ *   deterministic (identical inputs, identical bits; no floating-point atomics).
+ * Launch: one persistent kernel, launched with programmatic stream serialization; it touches no global memory before
+ * griddepcontrol.wait, so ordering against earlier work in the stream (a preceding er_quantize_pack included) is the
+ * usual one. */
 int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems,
                   const void* qweight, const void* scales, int64_t N, int group,
                   void* y, int64_t ldy_elems, int y_dtype,
