@@ -28,12 +28,3 @@ def whole_job_rate(units_per_rank: float, world: int, ms: float) -> float:
     if ms <= 0.0:
         raise ValueError("non-positive duration")
     return units_per_rank * world / ms / 1e6
-
-
-def shard_units(n_units: int, rank: int, world: int):
-    """Contiguous, balanced [begin, end) range of independent units (sequences / layers) owned by `rank`."""
-    if not (0 <= rank < world):
-        raise ValueError("rank out of range")
-    q, r = divmod(n_units, world)
-    begin = rank * q + min(rank, r)
-    return begin, begin + q + (1 if rank < r else 0)

@@ -1,5 +1,5 @@
 """The N > 1 (replica) path on CPU: two gloo ranks agree on max-over-ranks timings and rank 0 aggregates the
-whole-job rate; unit sharding is a partition.  (No GPU: the data path itself has no collective.)"""
+whole-job rate; `bench.py --gpus 2` starts its own ranks.  (No GPU: the data path itself has no collective.)"""
 import os
 import socket
 
@@ -56,10 +56,20 @@ def test_single_process_is_identity():
         multi.whole_job_rate(1.0, 1, 0.0)
 
 
-@pytest.mark.parametrize("n,world", [(64, 1), (64, 2), (64, 8), (7, 4), (3, 8), (0, 2)])
-def test_shard_units_is_a_balanced_partition(n, world):
-    ranges = [multi.shard_units(n, r, world) for r in range(world)]
-    assert ranges[0][0] == 0 and ranges[-1][1] == n
-    assert all(ranges[i][1] == ranges[i + 1][0] for i in range(world - 1))
-    sizes = [e - b for b, e in ranges]
-    assert max(sizes) - min(sizes) <= 1
+def test_bench_gpus_2_starts_two_ranks_itself():
+    # `python bench.py --gpus 2` without a torchrun environment must start the ranks itself (one process per GPU,
+    # rendezvous on 127.0.0.1); exercised on CPU with the reference arm, whose rank 0 prints the line and whose other
+    # ranks exit 0 without work
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--impl", "reference", "--steps", "1",
+                        "--warmup", "0"], capture_output=True, text=True, timeout=600, env=env, cwd=root)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1, r.stdout
+    out = json.loads(lines[0])
+    assert out["impl"] == "reference" and out["n_gpus"] == 2 and out["unit"] == "GB/s"
+    assert out["e2e"]["h2d_bytes_per_step"] == 0 and out["cpu_baseline"]["kind"] == "oracle"
