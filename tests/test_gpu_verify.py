@@ -150,7 +150,8 @@ def test_config4_full_batch_64(gamma):
     n_exact = _check_against_oracle(tgt, drf, toks, ua, us, acc, out)
     assert n_exact >= B // 2
     # statistical sanity of the workload: mean(n) + 1 ~ tau(alpha ~ 0.80, gamma)
-    assert abs(float(acc.float().mean()) + 1 - O.block_efficiency(0.80, gamma)) < 0.6
+    a = acc.float()
+    assert abs(float(a.mean()) + 1 - O.block_efficiency(0.80, gamma)) < 3.5 * float(a.std()) / np.sqrt(B) + 0.15
 
 
 def test_config2_maximum_batch_256_gamma_8():
