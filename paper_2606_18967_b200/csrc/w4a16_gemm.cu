@@ -1,33 +1,35 @@
 // w4a16_gemm.cu -- er_w4a16_gemm: the weight-quantized self-drafter's linear, Y = X . dequant(Wq)^T
 // (dense projections are ~90 % of tail decode latency and weight loading dominates at
 // small batch; L175: W4A16 weight-only kernel; L467: "on-the-fly dequantization and kernel-level overhead").
+// This file: the host entry point (validation, work plan, dispatch to the three kernels) and the tcgen05 kernel with
+// one fp32 accumulator per 128-k group (exact group scale), which serves M <= 16 -- except M <= 8 on plans without a
+// cluster (w4a16_gemm_small.cu) -- and 16 < M <= 64, and larger M where w4a16_gemm_large.cu is not preferred.
 //
-// sm_100a design, fourth version.  What the earlier ones taught
-// (profiles/r01_*): TMA / MMA issue must be warp-uniform code with one elected lane (otherwise the
-// compiler wraps every instruction in a per-lane loop); a closed ring of few TMEM buffers between separate
-// converter / MMA / read-back roles is bound by the round-trip latency of its mbarriers; and the nibble ->
-// bf16 conversion (7 logic-pipe operations per packed word, the logic pipe runs at half rate) is the
-// largest fixed cost, about 224 cycles per 128-k group and SM sub-partition, so it must never wait.
+// What the earlier versions taught (profiles/r01_*, r02_gemm.md): TMA / MMA issue must be warp-uniform code with one
+// elected lane; a closed ring of few TMEM buffers between separate converter / MMA / read-back roles is bound by the
+// round-trip latency of its mbarriers; the nibble -> bf16 conversion (7 logic-pipe operations per packed word, the
+// logic pipe runs at half rate) is the largest cost, ~224 cycles per 128-k group and SM sub-partition.
 //
 //   persistent   one CTA per SM; the (tile, 128-k group) units of the whole problem are dealt out as ONE
-//                contiguous range per CTA ("stream-K"): every CTA streams the same number of bytes.
+//                contiguous range per CTA (stream-K / tile split / thread-block cluster: w4a16_plan.cuh).
 //   swap-AB      the 128 weight rows of a tile are the M = 128 of tcgen05.mma, the padded batch is its N.
-//   warp 0       producer: per group ONE 8 KiB 1-D bulk copy of the packed block (ER_PACK_V2 keeps every
+//   warp 24      producer: per group ONE 8 KiB 1-D bulk copy of the packed block (ER_PACK_V2 keeps every
 //                [128 rows x 128 k] block contiguous and pre-swizzled), one 256-byte bulk copy of the group's
 //                scales and two SWIZZLE_128B TMA boxes of X [MPAD x 64 k], into a ring of up to 16 stages.
-//   warp 1       MMA issuer: tcgen05.mma.kind::f16, A (weights) from TENSOR MEMORY, B (= X tile) from shared
-//                memory, a fresh fp32 TMEM accumulator per group so the group scale is applied exactly.
-//   warps 4-27   three self-paced worker sets of 8 warps; set j owns the groups j, j+3, ... of the CTA's
-//                range, one A buffer and one accumulator in TMEM.  A thread owns HALF a weight row of the
-//                group.  Per group: 2 x LDS.128, nibble -> bf16 ((w >> 4t) & 0x000F000F | 0x43004300 = the
-//                pair 128 + u, one packed fma removes the 136), then the scale-accumulate of the set's
-//                PREVIOUS group (tcgen05.ld + fma: its MMAs had the whole conversion to finish), then
-//                tcgen05.st of the new A operand (the 4x expanded weights never touch shared memory) and
-//                an arrival on the set's a_full barrier.  The three sets interleave on the logic pipe.
+//   warps 25-26  MMA issuers: tcgen05.mma.kind::f16, A (weights) from TENSOR MEMORY, B (= X tile) from shared
+//                memory, a fresh fp32 TMEM accumulator per group so the group scale is applied exactly; at M <= 16
+//                eight more MMAs per group with a constant -136 tile remove the stored nibble's offset.
+//   warps 0-23   three self-paced worker sets of 8 warps; set j owns the groups j, j+3, ... of the CTA's range and
+//                its own (A operand, accumulator) buffers in TMEM (two pairs at M <= 16).  A thread owns HALF a
+//                weight row of the group.  Per group: wait for the stage (every warp on the mbarrier itself),
+//                2 x LDS.128, nibble -> bf16 ((w >> 4t) & 0x000F000F | 0x43004300 = the pair 128 + u; above M = 16
+//                one packed fma removes the 136), the scale-accumulate of the set's previous group (tcgen05.ld +
+//                fma: its MMAs had the whole conversion to finish), tcgen05.st of the new A operand (the 4x
+//                expanded weights never touch shared memory) and an arrival on the set's a_full barrier.
 //   output       at the end of a tile segment sets 1-2 hand their partial sums to set 0 through shared memory;
-//                a tile wholly owned by one CTA is stored directly, otherwise fp32 partials go to the workspace
-//                and the last CTA of the tile (ticket counter) adds them in ascending CTA order.
-//                Deterministic, no float atomics.
+//                a tile wholly owned by one CTA is stored directly; in cluster mode the CTAs of a tile add their
+//                sums through distributed shared memory; otherwise fp32 partials go to the workspace and the last
+//                CTA of the tile (ticket counter) adds them in ascending CTA order.  Deterministic.
 #include "w4a16_plan.cuh"
 
 namespace {
@@ -286,13 +288,12 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
     asm volatile("mov.u32 %0, %1;" : "=r"(full_addr) : "r"(smem_u32(full)));
     asm volatile("mov.u32 %0, %1;" : "=r"(done_addr) : "r"(smem_u32(&done[set * kBuf])));
     asm volatile("mov.u32 %0, %1;" : "=r"(afull_addr) : "r"(smem_u32(&a_full[set * kBuf])));
-    const bool poller = ((dw & 7) == 0);   // one warp of the set polls `full`, a named barrier releases the other
-                                           // seven (a blocked bar.sync costs no issue slots, a poll loop does)
+    // every warp waits on the mbarriers itself (try_wait suspends the warp in hardware): measured 1 % faster than one
+    // polling warp per set + a named barrier, and the warps of a set no longer wait for their slowest sibling
     const bool leader = (threadIdx.x == kSetWarp0 * 32);
     uint32_t a_t, d_t;
     asm volatile("mov.u32 %0, %1;" : "=r"(a_t) : "r"(tmem + lane_addr + kTmemA + set * kBuf * 64 + half * 32));
     asm volatile("mov.u32 %0, %1;" : "=r"(d_t) : "r"(tmem + lane_addr + C::kTmemD + set * kBuf * MPAD + half * CW));
-    const int bar_id = 1 + set;
 
     if (half == 0) {                       // the set's constant A tile (-136, -136), one lane quarter per warp; ordered
                                            // before the set's first MMA by its first a_full arrival
@@ -315,8 +316,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
 
     // scale-accumulate of the set's pending group: acc += scale * (sum over its 128 k of x * q)
     auto read_back = [&]() {
-      if (poller) mbar_wait_addr(done_addr + rbuf * 8, (pd >> rbuf) & 1);
-      named_bar_sync(bar_id, kSetThreads);
+      mbar_wait_addr(done_addr + rbuf * 8, (pd >> rbuf) & 1);
       pd ^= 1u << rbuf;
       tc_fence_after();
       uint32_t d[CW];
@@ -362,8 +362,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
 #pragma unroll
       for (int m = 0; m < CW; ++m) acc[m] = 0.f;
       for (; my < it_end; my += kSets) {
-        if (poller) mbar_wait_addr(full_addr + s * 8, ph);
-        named_bar_sync(bar_id, kSetThreads);
+        mbar_wait_addr(full_addr + s * 8, ph);
         {
           const uint32_t st = s * C::kStageBytes;
           if (C::kEpiFirst && npend == kBuf) read_back();
