@@ -186,12 +186,17 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
     }
     mbar_fence_init();
     if (lane == 0) tma_prefetch_desc(&map_x);
+    // the producer does not wait for the TENSOR-MEMORY allocation: it arrives on the prologue barrier and goes on to
+    // griddepcontrol.wait and its first loads (the ~0.3 us of the prologue are otherwise serialised behind the previous
+    // kernel's exit in every launch)
+    named_bar_arrive(15, kThreads);
+  } else {
+    if (warp == kMmaWarp0) tmem_alloc<kTmemCols>(tmem_slot);
+    tc_fence_before();
+    named_bar_sync(15, kThreads);
+    tc_fence_after();
   }
-  if (warp == kMmaWarp0) tmem_alloc<kTmemCols>(tmem_slot);
-  tc_fence_before();
-  __syncthreads();
-  tc_fence_after();
-  const uint32_t tmem = __shfl_sync(0xffffffffu, *tmem_slot, 0);
+  const uint32_t tmem = (warp == kProdWarp) ? 0u : __shfl_sync(0xffffffffu, *tmem_slot, 0);
   if constexpr (kClusterMode) {   // "I have started": waited for before the first remote shared-memory access
     if (p.cluster > 1) asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");
   }
@@ -200,6 +205,12 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   // scheduled as soon as SMs free up (it waits at its own griddepcontrol.wait).  (Issuing the first ring stages of
   // weights BEFORE the wait was measured and does not pay here: with one CTA per SM the next kernel's CTAs only
   // become resident when this kernel's exit, so there is nothing to overlap with -- profiles/r02_gemm.md.)
+  // The producer first asks L2 for the beginning of this CTA's weight stream (a contiguous byte range of ER_PACK_V2):
+  // safe even right behind a refresh, because L2 is the point of coherence and a prefetched line cannot be stale.
+  if (warp == kProdWarp && elect_one()) {
+    const int npf = n_it < 8 ? n_it : 8;          // 64 KB per SM: deeper prefetches measured slower (profiles/r02_gemm.md)
+    if (npf > 0) bulk_prefetch_l2(p.qweight + (size_t)gb * kWBytes, (uint32_t)npf * kWBytes);
+  }
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 

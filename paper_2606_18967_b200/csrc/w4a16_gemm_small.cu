@@ -50,6 +50,7 @@ constexpr int kProdWarp = kWorkerWarps;              // 20: the weight producer;
 constexpr int kThreads = (kWorkerWarps + 1 + kSets) * 32;   // 832
 constexpr int kXStages = 10;                         // ring of X / scale stages: two per set
 constexpr int kMaxWStages = 20;                      // ring of packed-weight stages: as deep as shared memory allows
+constexpr int kPrefetchGroups = 12;                  // 96 KB of weights asked from L2 before griddepcontrol.wait
 constexpr int kRedLd = 132;                          // row pitch of the shared reduction tile (bank-conflict free)
 
 template <int MB>
@@ -157,11 +158,20 @@ w4a16_small_kernel(const __grid_constant__ CUtensorMap map_x0, const __grid_cons
       tma_prefetch_desc(&map_x0);
       tma_prefetch_desc(&map_x1);
     }
+    named_bar_arrive(15, kThreads);   // the producer goes straight on to its first loads
+  } else {
+    named_bar_sync(15, kThreads);     // the barriers are initialised
   }
-  __syncthreads();
   // Programmatic dependent launch: the prologue above touched no global memory and may overlap the tail of the
   // previous kernel in the stream; from here on its results (X, the workspace) are needed.  The next kernel may be
   // scheduled as soon as SMs free up (it waits at its own griddepcontrol.wait).
+  // ... except that the weight producer first asks L2 for the beginning of this CTA's weight stream (a contiguous
+  // byte range of ER_PACK_V2): that hides part of the first DRAM round trip under the previous kernel's tail, and it is
+  // safe even right behind a refresh -- L2 is the point of coherence, a prefetched line cannot be stale.
+  if (warp == kProdWarp && elect_one()) {
+    const int npf = n_it < kPrefetchGroups ? n_it : kPrefetchGroups;
+    bulk_prefetch_l2(p.qweight + (size_t)gb * kWBytes, (uint32_t)npf * kWBytes);
+  }
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
