@@ -477,11 +477,12 @@ static LargePlan large_plan(int64_t M, int64_t N, int64_t K, int sms, int force_
   return best;
 }
 
-// true where the large-batch kernel gets whole tiles on at least ~45 % of the SMs (no split-K partial sums): there it
-// beats the exact per-group kernel from M > 64 on (profiles/r02_gemm.md); on long-K / few-tile shapes (`down`) the
-// exact kernel's stream-K stays
+// Where the large-batch kernel is preferred over the exact per-group kernel (measured on the 7B / 32B shapes,
+// profiles/r02_gemm.md): from M > 64 on, when it gets whole tiles on at least ~45 % of the SMs AND the reduction is not
+// long (K <= 8192).  On long-K / few-tile shapes (`down`: 28-40 tiles x 148-216 groups) whole tiles leave most of the
+// machine idle and its split-K partial tiles are up to 128 KB each: the exact kernel's stream-K is faster there.
 bool large_preferred(int64_t M, int64_t N, int64_t K) {
-  if (M <= 64) return false;
+  if (M <= 64 || K > 8192) return false;
   const LargePlan pl = large_plan(M, N, K, sm_count(), g_tune.force_ctas);
   return pl.unit_groups > 1 && (long long)pl.ctas * 100 >= (long long)sm_count() * 45;
 }
