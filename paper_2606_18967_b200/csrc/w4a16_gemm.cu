@@ -54,10 +54,10 @@ struct Cfg {
   static constexpr int kXBytes = MPAD * 128 * 2;           // two boxes of [MPAD x 64] bf16
   static constexpr int kStageBytes = ((kWBytes + kXBytes + kScaleBytes + 1023) / 1024) * 1024;
   static constexpr int kRedBytes = (kSets - 1) * MPAD * kTileN * 4;   // partial sums of sets 1.. handed to set 0
-  // cluster mode (M <= 16): up to 3 [MPAD x 128] fp32 slots that the other CTAs of the cluster write into rank 0;
+  // cluster mode (M <= 32): up to 3 [MPAD x 128] fp32 slots that the other CTAs of the cluster write into rank 0;
   // a region of their own, so the writers need not wait for rank 0's pipeline to drain (the ring depth is not
   // critical: 8 and 16 stages measure the same)
-  static constexpr int kSlotBytes = (MPAD == 16) ? 3 * MPAD * kTileN * 4 : 0;
+  static constexpr int kSlotBytes = (MPAD <= 32) ? 3 * MPAD * kTileN * 4 : 0;
   static constexpr int kFixed = kRedBytes + kSlotBytes + 1024 /*align slack*/ + 512 /*barriers*/;
   static constexpr int kStagesRaw = (kSmemLimit - kFixed) / kStageBytes;
   static constexpr int kStages = kStagesRaw > kMaxStages ? kMaxStages : kStagesRaw;
@@ -171,7 +171,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   const int gb = range_begin(p.uq, p.ur, p.split, cta) * ug;        // first global group index of this CTA
   const int ge = range_begin(p.uq, p.ur, p.split, cta + 1) * ug;
   const int n_it = (int)(ge - gb);
-  static_assert(!kClusterMode || MPAD == 16, "the host only uses clusters at M <= 16");
+  static_assert(!kClusterMode || MPAD <= 32, "the host only uses clusters at M <= 32");
   float cl_acc[kClusterMode ? C::kCW : 1];      // cluster mode: set 0's sum over this CTA's part of its tile ...
   int cl_tile = -1;                     // ... and the tile
 
@@ -633,10 +633,10 @@ Plan make_plan(int64_t M, int64_t N, int64_t K) {
       pl.ctas = pl.tiles * k;
     }
   }
-  // cluster mode (M <= 16): the parts of a tile are one thread-block cluster and reduce through distributed shared
+  // cluster mode (M <= 32): the parts of a tile are one thread-block cluster and reduce through distributed shared
   // memory.  The cluster size is limited by how many clusters of one-CTA-per-SM footprint the GPCs can hold at once.
   pl.cluster = 1;
-  if (tn.cluster && pl.mpad == 16 && pl.unit_groups == 1 && tn.force_ctas == 0 && pl.mchunks == 1) {
+  if (tn.cluster && pl.mpad <= 32 && pl.unit_groups == 1 && tn.force_ctas == 0 && pl.mchunks == 1) {
     for (int c = 4; c >= 2; --c) {
       if (c <= pl.G && max_active_clusters16(c) >= pl.tiles && pl.tiles * c * 10 >= ctas * 7) {
         pl.cluster = c;
@@ -793,7 +793,7 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
     return ER_ERR_CUDA;
   }
   if (pl.mpad == 16) return pl.cluster > 1 ? launch<16, true>(mx, gp, pl, s) : launch<16, false>(mx, gp, pl, s);
-  if (pl.mpad == 32) return launch<32, false>(mx, gp, pl, s);
+  if (pl.mpad == 32) return pl.cluster > 1 ? launch<32, true>(mx, gp, pl, s) : launch<32, false>(mx, gp, pl, s);
   return launch<64, false>(mx, gp, pl, s);
 }
 

@@ -387,3 +387,20 @@ def test_large_batch_kernel_exact_cases():
         xo[torch.arange(256), 1000 + torch.arange(256)] = 1.0
         y = er.w4a16_gemm(xo, qw2, sc2, out_dtype=torch.float32).cpu().numpy().astype(np.float64)
         assert np.array_equal(y, wd_bf16[:, 1000:1256].T)
+
+
+@pytest.mark.parametrize("mode", ["cluster", "stream_k"])
+@pytest.mark.parametrize("M", [17, 32])
+def test_partition_modes_at_m_17_to_32(mode, M):
+    # 16 < M <= 32 also runs the parts of a tile as a thread-block cluster (DSMEM reduction) on the small linears
+    N, K = 3584, 3584
+    w = I.weight_bf16(N, K, I.seed_of("modes32", "w"), device=DEV)
+    x = I.activation_bf16(M, K, I.seed_of("modes32", "x", M), device=DEV)
+    qw, sc = er.quantize_pack(w)
+    with er.dev_library() as lib:
+        lib.er_dev_gemm_tuning(5, 1 if mode == "cluster" else 0)
+        lib.er_dev_gemm_tuning(4, 0 if mode == "stream_k" else 1)
+        y1 = _sampled_columns_check(x, qw, sc, N, K, 9, mode)
+        y2 = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
+        torch.cuda.synchronize()
+        assert torch.equal(y1, y2)
