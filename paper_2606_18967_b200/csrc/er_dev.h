@@ -13,7 +13,8 @@ extern "C" {
  * 4: tile split (0/1); 5: thread-block-cluster mode (0/1); 6: M <= 8 through the warp-level-MMA kernel (0/1);
  * 7: the pre-scaled large-batch kernel: 0 never, 1 where the plan prefers it (default), 2 for every M > 16. */
 int er_dev_gemm_tuning(int key, int value);
-/* CTAs per sequence of er_spec_verify: 0 = automatic, or 1 / 2 / 4 / 8. */
+/* CTAs per sequence of er_spec_verify: 0 = automatic, or 1 / 2 / 4 / 8.  16 / 17: the shared-memory ring kernel
+ * where it applies (default) / the register-path kernel for every input. */
 int er_dev_verify_cluster(int cluster);
 
 #ifdef __cplusplus

@@ -117,17 +117,25 @@ __device__ __forceinline__ float warp_sum(float x) {
   return x;
 }
 
+// A row's softmax as one fma and one ex2 per logit: p(v) = 2^(l_v * scale + bias), bias = -m * scale - log2(sum_v
+// 2^((l_v - m) * scale)) for the row's reference m.  (Probability inputs do not use it.)
 struct RowStats {
-  float max;      // max logit of the row
-  float inv_sum;  // 1 / sum_v exp((l - max) / T)
+  float bias;
 };
+__device__ __forceinline__ RowStats row_stats_of(float m, float inv_sum, float scale) {
+  return RowStats{fmaf(-m, scale, log2f(inv_sum))};
+}
+
+constexpr int kMaxRows = 33;         // gamma <= 16: rows t_0, d_0, t_1, d_1, ..., t_gamma
+constexpr int kMaxDepth = 12;        // stages of the shared-memory ring (ring kernel)
 
 struct Shared {
-  double xmass[2][kMaxCluster];    // [parity][rank]: residual mass of every CTA's range
-  float4 wstat[17][kWarps];        // [position][warp]: per-warp (max_t, sum_t, max_d, sum_d) of this CTA's range
-  float4 xall[kMaxCluster][17];    // [rank][position]: per-CTA statistics of every CTA of the cluster
-  float4 stat[17];                 // [position]: (max_t, 1/sum_t, max_d, 1/sum_d) over the whole vocabulary
-  float px[16], qx[16], ua[16];    // target / draft value at the drafted token and the uniform, per position
+  double xmass[2][kMaxCluster];      // [parity][rank]: residual mass of every CTA's range
+  float2 wstat[kMaxRows][32];        // [row][warp]: per-warp (max, sum) of this CTA's range of the row
+  float2 xall[kMaxCluster][kMaxRows];  // [rank][row]: per-CTA statistics of every CTA of the cluster
+  float4 stat[17];                   // [position]: (max_t, 1/sum_t, max_d, 1/sum_d) over the whole vocabulary
+  float px[16], qx[16], ua[16];      // target / draft value at the drafted token and the uniform, per position
+  uint64_t full[kMaxDepth], empty[kMaxDepth];   // ring kernel: stage landed / stage consumed
   int token;
   int flag;
 };
@@ -147,14 +155,38 @@ __device__ __forceinline__ void cluster_started(ClusterCtx& cx) {
   cx.started = true;
 }
 
-// Online softmax statistics of one lane: running maximum m, sum s of 2^((l - m) * scale), nm = -m * scale.
-// run2 (bf16 rows only) is the running maximum on the packed words, lane-wise over the two halves.
+// Online softmax statistics of one lane: a REFERENCE logit m (the maximum of some chunk seen so far), four partial
+// sums s[] of 2^((l - m) * scale) and nm = -m * scale.  The reference is raised lazily (the trick of recent
+// attention kernels): only when a chunk holds a logit above thr = m + kMargin / scale, i.e. when a term would
+// exceed 2^kMargin -- with fp32 sums of at most 2^20 terms that is far from overflow, and the result is the same
+// (reference, sum) pair algebra as an exact running maximum.  After the first chunk of a row the raise is
+// practically never taken, so the loop is: maximum of the chunk on the packed words, one compare, then
+// unpack / fma / ex2 / add per logit.
+constexpr float kMargin = 32.f;
+
 struct Acc {
-  float m, s, nm;
-  uint32_t run2;
-  __device__ __forceinline__ void init() { m = kNegInf; s = 0.f; nm = 0.f; run2 = 0xFF80FF80u; }   // (-inf, -inf)
+  float m, nm, s[4];
+  float thr;          // float rows: raise when a logit exceeds this
+  uint32_t thr2;      // bf16 rows: the same as packed bf16x2 (rounded down)
+  __device__ __forceinline__ void init() {
+    m = kNegInf; nm = 0.f; thr = __uint_as_float(0xFF800000u); thr2 = 0xFF80FF80u;   // -inf: the first finite chunk raises
+#pragma unroll
+    for (int i = 0; i < 4; ++i) s[i] = 0.f;
+  }
+  __device__ __forceinline__ float sum() const { return (s[0] + s[1]) + (s[2] + s[3]); }
+  // cm = the maximum of the chunk that tripped the threshold: it becomes the reference
   __device__ __forceinline__ void raise(float cm, float scale) {
-    if (cm > m) { s *= ex2_fast((m - cm) * scale); m = cm; nm = -cm * scale; }
+    const float f = ex2_fast((m - cm) * scale);     // m = -3e38 at first: f = 0 and the sums are 0 anyway
+#pragma unroll
+    for (int i = 0; i < 4; ++i) s[i] *= f;
+    m = cm;
+    nm = -cm * scale;
+    thr = cm + kMargin / scale;
+    uint32_t b = __float_as_uint(thr);              // bf16 not above thr: truncation rounds a negative value up,
+    uint32_t h = b >> 16;                           // so step one further down there
+    if ((b & 0x80000000u) && (b & 0xFFFFu)) h += 1;
+    if ((b & 0x7F800000u) == 0x7F800000u) h = 0x7F7Fu;   // thr overflowed (tiny scale): largest finite bf16
+    thr2 = h | (h << 16);
   }
 };
 
@@ -163,51 +195,87 @@ __device__ __forceinline__ uint32_t max_bf16x2(uint32_t a, uint32_t b) {
   asm("max.bf16x2 %0, %1, %2;" : "=r"(d) : "r"(a), "r"(b));
   return d;
 }
+// true if either half of a exceeds the same half of b
+__device__ __forceinline__ bool any_gt_bf16x2(uint32_t a, uint32_t b) {
+  uint32_t r;
+  asm("{\n\t.reg .pred p, q;\n\t"
+      "setp.gt.bf16x2 p|q, %1, %2;\n\t"
+      "or.pred p, p, q;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}\n"
+      : "=r"(r)
+      : "r"(a), "r"(b));
+  return r != 0;
+}
 
+// N chunks of 8 logits of one row -> the lane's statistics.  A chunk that does not exist is passed as all -inf:
+// it never trips the threshold, and its terms are 2^(-inf) = 0 (nm is finite, so no inf - inf).
 template <typename T>
 struct Accum;
 template <>
 struct Accum<float> {
-  static __device__ __forceinline__ void add(const Load8<float>::Raw& r, Acc& a, float scale) {
-    float f[8];
-    Load8<float>::expand(r, f);
-    float cm = fmaxf(fmaxf(fmaxf(f[0], f[1]), fmaxf(f[2], f[3])), fmaxf(fmaxf(f[4], f[5]), fmaxf(f[6], f[7])));
-    a.raise(cm, scale);
-    if (a.m > kNegInf) {   // masked (-inf) logits before any finite one add nothing (and -m * scale would
-                           // overflow: fma(-inf, scale, +inf) is NaN)
-      float s0 = 0.f, s1 = 0.f;
+  static __device__ __forceinline__ Load8<float>::Raw neg_inf() {
+    const float x = __uint_as_float(0xFF800000u);
+    Load8<float>::Raw r;
+    r.a = make_float4(x, x, x, x);
+    r.b = r.a;
+    return r;
+  }
+  template <int N>
+  static __device__ __forceinline__ void add(const Load8<float>::Raw (&r)[N], Acc& a, float scale) {
+    float cm = __uint_as_float(0xFF800000u);
 #pragma unroll
-      for (int i = 0; i < 8; i += 2) {
-        s0 += ex2_fast(fmaf(f[i], scale, a.nm));
-        s1 += ex2_fast(fmaf(f[i + 1], scale, a.nm));
-      }
-      a.s += s0 + s1;
+    for (int j = 0; j < N; ++j)
+      cm = fmaxf(cm, fmaxf(fmaxf(fmaxf(r[j].a.x, r[j].a.y), fmaxf(r[j].a.z, r[j].a.w)),
+                           fmaxf(fmaxf(r[j].b.x, r[j].b.y), fmaxf(r[j].b.z, r[j].b.w))));
+    if (cm > a.thr) a.raise(cm, scale);
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+      a.s[0] += ex2_fast(fmaf(r[j].a.x, scale, a.nm)) + ex2_fast(fmaf(r[j].b.x, scale, a.nm));
+      a.s[1] += ex2_fast(fmaf(r[j].a.y, scale, a.nm)) + ex2_fast(fmaf(r[j].b.y, scale, a.nm));
+      a.s[2] += ex2_fast(fmaf(r[j].a.z, scale, a.nm)) + ex2_fast(fmaf(r[j].b.z, scale, a.nm));
+      a.s[3] += ex2_fast(fmaf(r[j].a.w, scale, a.nm)) + ex2_fast(fmaf(r[j].b.w, scale, a.nm));
     }
   }
 };
 template <>
 struct Accum<__nv_bfloat16> {
-  static __device__ __forceinline__ void add(const Load8<__nv_bfloat16>::Raw& r, Acc& a, float scale) {
-    const uint32_t n2 = max_bf16x2(max_bf16x2(max_bf16x2(r.a.x, r.a.y), max_bf16x2(r.a.z, r.a.w)), a.run2);
-    if (n2 != a.run2) {    // rare after the first few segments
-      a.run2 = n2;
-      a.raise(fmaxf(__uint_as_float(n2 << 16), __uint_as_float(n2 & 0xFFFF0000u)), scale);
-    }
-    if (a.m > kNegInf) {
-      const uint32_t w[4] = {r.a.x, r.a.y, r.a.z, r.a.w};
-      float s0 = 0.f, s1 = 0.f;
+  static __device__ __forceinline__ Load8<__nv_bfloat16>::Raw neg_inf() {
+    Load8<__nv_bfloat16>::Raw r;
+    r.a = make_uint4(0xFF80FF80u, 0xFF80FF80u, 0xFF80FF80u, 0xFF80FF80u);
+    return r;
+  }
+  template <int N>
+  static __device__ __forceinline__ void add(const Load8<__nv_bfloat16>::Raw (&r)[N], Acc& a, float scale) {
+    uint32_t n2 = max_bf16x2(max_bf16x2(r[0].a.x, r[0].a.y), max_bf16x2(r[0].a.z, r[0].a.w));
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        s0 += ex2_fast(fmaf(__uint_as_float(w[i] << 16), scale, a.nm));
-        s1 += ex2_fast(fmaf(__uint_as_float(w[i] & 0xFFFF0000u), scale, a.nm));
-      }
-      a.s += s0 + s1;
+    for (int j = 1; j < N; ++j)
+      n2 = max_bf16x2(n2, max_bf16x2(max_bf16x2(r[j].a.x, r[j].a.y), max_bf16x2(r[j].a.z, r[j].a.w)));
+    if (any_gt_bf16x2(n2, a.thr2))
+      a.raise(fmaxf(__uint_as_float(n2 << 16), __uint_as_float(n2 & 0xFFFF0000u)), scale);
+#pragma unroll
+    for (int j = 0; j < N; ++j) {
+      a.s[0] += ex2_fast(fmaf(__uint_as_float(r[j].a.x << 16), scale, a.nm));
+      a.s[1] += ex2_fast(fmaf(__uint_as_float(r[j].a.x & 0xFFFF0000u), scale, a.nm));
+      a.s[2] += ex2_fast(fmaf(__uint_as_float(r[j].a.y << 16), scale, a.nm));
+      a.s[3] += ex2_fast(fmaf(__uint_as_float(r[j].a.y & 0xFFFF0000u), scale, a.nm));
+      a.s[0] += ex2_fast(fmaf(__uint_as_float(r[j].a.z << 16), scale, a.nm));
+      a.s[1] += ex2_fast(fmaf(__uint_as_float(r[j].a.z & 0xFFFF0000u), scale, a.nm));
+      a.s[2] += ex2_fast(fmaf(__uint_as_float(r[j].a.w << 16), scale, a.nm));
+      a.s[3] += ex2_fast(fmaf(__uint_as_float(r[j].a.w & 0xFFFF0000u), scale, a.nm));
     }
   }
 };
 
+// The lanes' statistics of one row -> one (reference, sum) of the warp (no CTA barrier per row): the largest
+// reference, then the sum of the rescaled sums.
+__device__ __forceinline__ void warp_row_stat(const Acc& a, float scale, float2& out) {
+  const float wm = warp_max(a.m);
+  const float ws = warp_sum((a.m > kNegInf) ? a.sum() * ex2_fast((a.m - wm) * scale) : 0.f);
+  if ((threadIdx.x & 31) == 0) out = make_float2(wm, ws);
+}
+
 // Softmax statistics of one target row and (optionally) one draft row over this CTA's segment range, reduced to
-// one entry per warp in sh.wstat[pos].  Warp w takes the local segments (w - rot) mod kWarps, + kWarps, ...;
+// one entry per warp in sh.wstat[2 pos] and sh.wstat[2 pos + 1].  Warp w takes the local segments (w - rot) mod kWarps, + kWarps, ...;
 // rot advances with the position by the size of the ragged remainder, so the extra segment of a row goes to
 // different warps in consecutive rows.
 template <typename T>
@@ -227,26 +295,18 @@ __device__ void row_stats(const T* trow, const T* drow, int V, bool vec, float s
 #pragma unroll
     for (int j = 0; j < NB; ++j) {           // all loads of the batch first: they overlap in flight
       const int v0 = (cx.seg_lo + s0 + j * kWarps) * kSeg + lane * kPerThread;
+      rt[j] = Accum<T>::neg_inf();
+      rd[j] = rt[j];
       if (s0 + j * kWarps < nloc && v0 < V) {
         rt[j] = Load8<T>::load(trow, v0, V, vec, kNegInf);
         if (drow) rd[j] = Load8<T>::load(drow, v0, V, vec, kNegInf);
       }
     }
-#pragma unroll
-    for (int j = 0; j < NB; ++j) {
-      const int v0 = (cx.seg_lo + s0 + j * kWarps) * kSeg + lane * kPerThread;
-      if (s0 + j * kWarps < nloc && v0 < V) {
-        Accum<T>::add(rt[j], at, scale);
-        if (drow) Accum<T>::add(rd[j], ad, scale);
-      }
-    }
+    Accum<T>::add(rt, at, scale);
+    if (drow) Accum<T>::add(rd, ad, scale);
   }
-  // warp level only (no CTA barrier per position): max, then the sum of the rescaled partial sums
-  const float wm_t = warp_max(at.m), wm_d = warp_max(ad.m);
-  const float st_ = (at.m > kNegInf) ? at.s * ex2_fast((at.m - wm_t) * scale) : 0.f;
-  const float sd_ = (ad.m > kNegInf) ? ad.s * ex2_fast((ad.m - wm_d) * scale) : 0.f;
-  const float ws_t = warp_sum(st_), ws_d = warp_sum(sd_);
-  if (lane == 0) sh.wstat[pos][warp] = make_float4(wm_t, ws_t, wm_d, ws_d);
+  warp_row_stat(at, scale, sh.wstat[2 * pos][warp]);
+  if (drow) warp_row_stat(ad, scale, sh.wstat[2 * pos + 1][warp]);
 }
 
 // (max, sum) pairs a and b of two disjoint parts of a row -> the pair of their union
@@ -258,28 +318,31 @@ __device__ __forceinline__ void merge_stat(float& m, float& s, float m2, float s
   s = a + b;
 }
 
-// After row_stats of positions 0..npos-1: combine the warps of a position (one warp per position, a fixed
+// After the statistics of rows 0 .. 2 gamma: combine the nw warps that wrote a row (one warp per row, a fixed
 // shuffle tree), exchange over the cluster through distributed shared memory, combine ranks (in order).  Every
 // CTA ends with the same sh.stat[].
-__device__ void combine_stats(int npos, float scale, Shared& sh, ClusterCtx& cx) {
+__device__ void combine_stats(int gamma, int nw, float scale, Shared& sh, ClusterCtx& cx) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int nrows = 2 * gamma + 1, warps = (int)(blockDim.x >> 5);
   cg::cluster_group cluster = cg::this_cluster();
   cluster_started(cx);
   __syncthreads();
-  for (int p = warp; p < npos; p += kWarps) {
-    const float4 v = (lane < kWarps) ? sh.wstat[p][lane] : make_float4(kNegInf, 0.f, kNegInf, 0.f);
-    const float mt = warp_max(v.x), md = warp_max(v.z);
-    const float st = warp_sum(v.x > kNegInf ? v.y * exp2f((v.x - mt) * scale) : 0.f);
-    const float sd = warp_sum(v.z > kNegInf ? v.w * exp2f((v.z - md) * scale) : 0.f);
-    if (lane < cx.size) *cluster.map_shared_rank(&sh.xall[cx.rank][p], lane) = make_float4(mt, st, md, sd);
+  for (int r = warp; r < nrows; r += warps) {
+    const float2 v = (lane < nw) ? sh.wstat[r][lane] : make_float2(kNegInf, 0.f);
+    const float m = warp_max(v.x);
+    const float sm = warp_sum(v.x > kNegInf ? v.y * exp2f((v.x - m) * scale) : 0.f);
+    if (lane < cx.size) *cluster.map_shared_rank(&sh.xall[cx.rank][r], lane) = make_float2(m, sm);
   }
   cluster.sync();
-  if (tid < npos) {
+  if (tid <= gamma) {
     float mt = kNegInf, st = 0.f, md = kNegInf, sd = 0.f;
     for (int c = 0; c < cx.size; ++c) {
-      const float4 v = sh.xall[c][tid];
+      const float2 v = sh.xall[c][2 * tid];
       merge_stat(mt, st, v.x, v.y, scale);
-      merge_stat(md, sd, v.z, v.w, scale);
+      if (tid < gamma) {
+        const float2 u = sh.xall[c][2 * tid + 1];
+        merge_stat(md, sd, u.x, u.y, scale);
+      }
     }
     sh.stat[tid] = make_float4(mt, __fdiv_rn(1.0f, st), md, sd > 0.f ? __fdiv_rn(1.0f, sd) : 0.f);
   }
@@ -295,17 +358,15 @@ __device__ __forceinline__ void weights8_raw(const typename Load8<T>::Raw& rp, c
   float p[8];
   Load8<T>::expand(rp, p);
   if (kLogits) {
-    const float nt = -st.max * scale;
 #pragma unroll
-    for (int i = 0; i < 8; ++i) p[i] = ex2_fast(fmaf(p[i], scale, nt)) * st.inv_sum;
+    for (int i = 0; i < 8; ++i) p[i] = ex2_fast(fmaf(p[i], scale, st.bias));
   }
   if (use_q) {
     float q[8];
     Load8<T>::expand(rq, q);
     if (kLogits) {
-      const float nd = -sd.max * scale;
 #pragma unroll
-      for (int i = 0; i < 8; ++i) q[i] = ex2_fast(fmaf(q[i], scale, nd)) * sd.inv_sum;
+      for (int i = 0; i < 8; ++i) q[i] = ex2_fast(fmaf(q[i], scale, sd.bias));
     }
 #pragma unroll
     for (int i = 0; i < 8; ++i) w[i] = fmaxf(0.f, p[i] - q[i]);
@@ -323,14 +384,12 @@ __device__ __forceinline__ void weights8(const T* trow, const T* drow, int v0, i
   weights8_raw<T, kLogits>(rp, rq, scale, st, sd, use_q, w);
 }
 
-// Inverse-CDF draw over w in vocab order: token = min{v : C(v) > r R}.  Returns -1 in every CTA of the cluster
-// if R == 0; otherwise the token in the CTA whose segment range holds the threshold and -2 in the others.
+// Inverse-CDF draw over w in vocab order, level 1: the sums of this CTA's 256-token segments, one warp each.
 template <typename T, bool kLogits>
-__device__ int draw_token(const T* trow, const T* drow, int V, bool vec, float scale, const RowStats& st,
-                          const RowStats& sd, bool use_q, float r, Shared& sh, ClusterCtx& cx, float* seg_sums) {
+__device__ void draw_segment_sums(const T* trow, const T* drow, int V, bool vec, float scale, const RowStats& st,
+                                  const RowStats& sd, bool use_q, const ClusterCtx& cx, float* seg_sums) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int nloc = cx.seg_hi - cx.seg_lo;
-  // level 1: sums of this CTA's 256-token segments, one warp each
   constexpr int NB = Load8<T>::kBatch;
   const float fill = kLogits ? kNegInf : 0.f;
   for (int s0 = warp; s0 < nloc; s0 += NB * kWarps) {
@@ -358,6 +417,17 @@ __device__ int draw_token(const T* trow, const T* drow, int V, bool vec, float s
       }
     }
   }
+}
+
+// Levels 2 and 3 of the draw, once seg_sums holds this CTA's segment sums: token = min{v : C(v) > r R}.  Returns -1
+// in every CTA of the cluster if R == 0; otherwise the token in the CTA whose segment range holds the threshold
+// and -2 in the others.
+template <typename T, bool kLogits>
+__device__ int draw_finish(const T* trow, const T* drow, int V, bool vec, float scale, const RowStats& st,
+                           const RowStats& sd, bool use_q, float r, Shared& sh, ClusterCtx& cx,
+                           const float* seg_sums) {
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int nloc = cx.seg_hi - cx.seg_lo;
   __syncthreads();
   // level 2a (warp 0): fp64 prefix over the segments in vocab order -- lane l sums the block [l blk, (l+1) blk)
   // sequentially, then an inclusive scan over the lanes; the last lane's value is this CTA's mass, published to
@@ -467,6 +537,44 @@ __device__ int draw_token(const T* trow, const T* drow, int V, bool vec, float s
   return sh.token;
 }
 
+// The accept tests: n = number of drafted tokens accepted before the first rejection, decided by
+// one thread from sh.px / qx / ua (and sh.stat for logits); every CTA of the cluster takes the same decisions from
+// the same numbers.  u q < p is evaluated in fp32 (V3).
+template <bool kLogits>
+__device__ int accept_prefix(int gamma, float scale, Shared& sh) {
+  if (threadIdx.x == 0) {
+    int k = 0;
+    for (; k < gamma; ++k) {
+      float p = sh.px[k], q = sh.qx[k];
+      if (kLogits) {
+        const float4 v = sh.stat[k];
+        p = exp2f((p - v.x) * scale) * v.y;
+        q = exp2f((q - v.z) * scale) * v.w;
+      }
+      const float lhs = __fmul_rn(sh.ua[k], q);
+      if (!(lhs < p)) break;
+    }
+    sh.flag = k;
+  }
+  __syncthreads();
+  return sh.flag;
+}
+
+// accept_count[b] and out_tokens[b][0 .. gamma], by the CTA that owns the draw (tok >= 0).
+__device__ void write_outputs(int tok, int n, int b, int gamma, int V, const int32_t* xs, const ClusterCtx& cx,
+                              int32_t* accept_count, int32_t* out_tokens) {
+  if (tok == -1) tok = (cx.rank == 0) ? V - 1 : -2;  // all-zero target row: outside the contract, stay memory-safe
+  if (tok == -2) return;                             // another CTA of the cluster owns the draw and the outputs
+  const int tid = threadIdx.x;
+  if (tid == 0) accept_count[b] = n;
+  if (tid <= gamma) {
+    int32_t o = -1;
+    if (tid < n) o = xs[tid];
+    else if (tid == n) o = tok;
+    out_tokens[(size_t)b * (gamma + 1) + tid] = o;
+  }
+}
+
 template <typename T, bool kLogits>
 __global__ void __launch_bounds__(kThreads, 1)
 spec_verify_kernel(const T* __restrict__ target, const T* __restrict__ draft, float scale,
@@ -505,43 +613,260 @@ spec_verify_kernel(const T* __restrict__ target, const T* __restrict__ draft, fl
   if (kLogits) {
     for (int i = 0; i <= gamma; ++i)
       row_stats<T>(tgt + (size_t)i * V, i < gamma ? drf + (size_t)i * V : nullptr, V, vec, scale, sh, cx, i);
-    combine_stats(gamma + 1, scale, sh, cx);
+    combine_stats(gamma, kWarps, scale, sh, cx);
   }
-  if (tid == 0) {              // every CTA of the cluster takes the same decisions from the same numbers
-    int k = 0;
-    for (; k < gamma; ++k) {
-      float p = sh.px[k], q = sh.qx[k];
-      if (kLogits) {
-        const float4 v = sh.stat[k];
-        p = exp2f((p - v.x) * scale) * v.y;
-        q = exp2f((q - v.z) * scale) * v.w;
-      }
-      const float lhs = __fmul_rn(sh.ua[k], q);
-      if (!(lhs < p)) break;
-    }
-    sh.flag = k;
-  }
-  __syncthreads();
-  const int n = sh.flag;
-  RowStats st{0.f, 1.f}, sd{0.f, 1.f};
+  const int n = accept_prefix<kLogits>(gamma, scale, sh);
+  RowStats st{0.f}, sd{0.f};
   if (kLogits) {
     const float4 v = sh.stat[n];
-    st.max = v.x; st.inv_sum = v.y; sd.max = v.z; sd.inv_sum = v.w;
+    st = row_stats_of(v.x, v.y, scale);
+    if (n < gamma) sd = row_stats_of(v.z, v.w, scale);
   }
   const T* trow = tgt + (size_t)n * V;
   const T* drow = (n < gamma) ? drf + (size_t)n * V : nullptr;
   const float r = u_sample[b];
-  int tok = draw_token<T, kLogits>(trow, drow, V, vec, scale, st, sd, n < gamma, r, sh, cx, seg_sums);
-  if (tok == -1) tok = draw_token<T, kLogits>(trow, nullptr, V, vec, scale, st, sd, false, r, sh, cx, seg_sums);
-  if (tok == -1) tok = (cx.rank == 0) ? V - 1 : -2;  // all-zero target row: outside the contract, stay memory-safe
-  if (tok == -2) return;                             // another CTA of the cluster owns the draw and the outputs
-  if (tid == 0) accept_count[b] = n;
-  if (tid <= gamma) {
-    int32_t o = -1;
-    if (tid < n) o = xs[tid];
-    else if (tid == n) o = tok;
-    out_tokens[(size_t)b * (gamma + 1) + tid] = o;
+  draw_segment_sums<T, kLogits>(trow, drow, V, vec, scale, st, sd, n < gamma, cx, seg_sums);
+  int tok = draw_finish<T, kLogits>(trow, drow, V, vec, scale, st, sd, n < gamma, r, sh, cx, seg_sums);
+  if (tok == -1) {   // no residual mass: draw from the target row itself
+    draw_segment_sums<T, kLogits>(trow, nullptr, V, vec, scale, st, sd, false, cx, seg_sums);
+    tok = draw_finish<T, kLogits>(trow, nullptr, V, vec, scale, st, sd, false, r, sh, cx, seg_sums);
   }
+  write_outputs(tok, n, b, gamma, V, xs, cx, accept_count, out_tokens);
+}
+
+// ---------------------------------------------------------------------------------------------------------------
+// Ring kernel (logits whose rows are 16-byte multiples: every paper-shaped workload).  The loads of the sweep are
+// taken off the compute warps: one producer lane streams the CTA's slice of row after row through a 192 KB ring
+// of shared-memory stages with cp.async.bulk (a stage = 32 consecutive segments of one row), kCons consumer warps
+// take two segments of every stage each.  The ring never drains at a row boundary, so the special-function unit
+// and HBM overlap instead of taking turns (the register path above waits for a DRAM round trip per batch of
+// loads).  The draw pass goes through the same ring, a stage = 16 segments of the target row + the same 16 of the
+// draft row.
+constexpr int kCons = 31;                       // consumer warps
+constexpr int kRingThreads = (kCons + 1) * 32;  // + the producer warp
+constexpr int kSPW = 2;                         // segments per consumer warp and sweep stage
+constexpr int kStageSegs = kCons * kSPW;
+constexpr int kRingBytes = 192 * 1024;
+
+template <typename T>
+struct Ring {
+  static constexpr int kSegBytes = kSeg * (int)sizeof(T);
+  static constexpr int kStageBytes = kStageSegs * kSegBytes;
+  static constexpr int kDepth = kRingBytes / kStageBytes;
+  static_assert(kDepth >= 2 && kDepth <= kMaxDepth, "ring depth");
+  static_assert(kStageBytes % 32 == 0, "the two halves of a draw stage are 16-byte aligned");
+};
+
+// Position in the ring, stepped identically by the producer lane and by every consumer warp: slot and the parity
+// of the slot's current use.  A consumer waits on full[slot] with `phase`; the producer waits on empty[slot] with
+// phase ^ 1 (on a fresh barrier that is the already-completed "previous" phase, so the first round passes).
+template <int kDepth>
+struct Pipe {
+  uint32_t slot = 0, phase = 0;
+  __device__ __forceinline__ void step() {
+    if (++slot == kDepth) { slot = 0; phase ^= 1; }
+  }
+};
+
+__device__ __forceinline__ void bulk_load_plain(void* smem_dst, const void* gsrc, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   er::smem_u32(smem_dst)),
+               "l"(gsrc), "r"(bytes), "r"(er::smem_u32(bar))
+               : "memory");
+}
+
+// the lanes of a float row's last chunk that lie beyond V were not copied: give them the fill value
+__device__ __forceinline__ void clip_tail(Load8<float>::Raw& r, int v0, int V, float fill) {
+  if (v0 + 8 > V) {
+    float* f = reinterpret_cast<float*>(&r);
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+      if (v0 + i >= V) f[i] = fill;
+  }
+}
+__device__ __forceinline__ void clip_tail(Load8<__nv_bfloat16>::Raw&, int, int, float) {}   // V % 8 == 0 here
+
+// Producer lane: the bytes [seg_lo kSeg, min(seg_hi kSeg, V)) of row_a -- and, if row_b is given, the same bytes of
+// row_b -- in stages of `segs` segments into consecutive ring slots: row_a into the first half of a slot
+// (or all of it), row_b into the second half.  A slot is refilled once every consumer warp has released it.
+template <typename T>
+__device__ __forceinline__ void produce_rows(unsigned char* ring, Shared& sh, Pipe<Ring<T>::kDepth>& pp,
+                                             const T* row_a, const T* row_b, int V, const ClusterCtx& cx, int segs) {
+  using R = Ring<T>;
+  const long long lo = (long long)cx.seg_lo * kSeg;
+  const long long hi = min((long long)cx.seg_hi * kSeg, (long long)V);
+  const long long total = (hi - lo) * (long long)sizeof(T);
+  const long long step = (long long)segs * R::kSegBytes;
+  const unsigned char* src_a = reinterpret_cast<const unsigned char*>(row_a + lo);
+  const unsigned char* src_b = reinterpret_cast<const unsigned char*>(row_b + lo);
+  for (long long off = 0; off < total; off += step, pp.step()) {
+    er::mbar_wait(&sh.empty[pp.slot], pp.phase ^ 1);
+    const uint32_t bytes = (uint32_t)min(step, total - off);
+    unsigned char* dst = ring + (size_t)pp.slot * R::kStageBytes;
+    er::mbar_arrive_expect_tx(&sh.full[pp.slot], row_b ? 2 * bytes : bytes);
+    bulk_load_plain(dst, src_a + off, bytes, &sh.full[pp.slot]);
+    if (row_b) bulk_load_plain(dst + R::kStageBytes / 2, src_b + off, bytes, &sh.full[pp.slot]);
+  }
+}
+
+// Consumer warps: online statistics of one row from the ring; sh.wstat[row][warp].  The segments of a stage are
+// dealt to the warps in a rotation that advances with the row by the size of the ragged last stage.
+template <typename T>
+__device__ __forceinline__ void consume_row_stats(const unsigned char* ring, Shared& sh, Pipe<Ring<T>::kDepth>& pp,
+                                                  int row, int V, float scale, const ClusterCtx& cx) {
+  using R = Ring<T>;
+  using Raw = typename Load8<T>::Raw;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nloc = cx.seg_hi - cx.seg_lo;
+  const int nst = (nloc + kStageSegs - 1) / kStageSegs;
+  // stages in which every segment exists and lies wholly below V: no validity tests there
+  const int nfull = (int)min((long long)nloc, (long long)V / kSeg - cx.seg_lo) / kStageSegs;
+  const int rot = (row * (nloc % kStageSegs)) % kStageSegs;
+  int jj[kSPW];
+  uint32_t off[kSPW];
+#pragma unroll
+  for (int j = 0; j < kSPW; ++j) {
+    jj[j] = warp * kSPW + j + rot;
+    if (jj[j] >= kStageSegs) jj[j] -= kStageSegs;
+    off[j] = (uint32_t)(jj[j] * R::kSegBytes + lane * kPerThread * (int)sizeof(T));
+  }
+  Acc a;
+  a.init();
+  for (int k = 0; k < nst; ++k, pp.step()) {
+    er::mbar_wait(&sh.full[pp.slot], pp.phase);
+    const unsigned char* stage = ring + (size_t)pp.slot * R::kStageBytes;
+    Raw r[kSPW];
+    if (k < nfull) {
+#pragma unroll
+      for (int j = 0; j < kSPW; ++j) r[j] = *reinterpret_cast<const Raw*>(stage + off[j]);
+    } else {
+#pragma unroll
+      for (int j = 0; j < kSPW; ++j) {
+        const int sg = k * kStageSegs + jj[j];
+        const int v0 = (cx.seg_lo + sg) * kSeg + lane * kPerThread;
+        r[j] = Accum<T>::neg_inf();
+        if (sg < nloc && v0 < V) {
+          r[j] = *reinterpret_cast<const Raw*>(stage + off[j]);
+          clip_tail(r[j], v0, V, kNegInf);
+        }
+      }
+    }
+    Accum<T>::add(r, a, scale);
+    __syncwarp();
+    if (lane == 0) er::mbar_arrive(&sh.empty[pp.slot]);
+  }
+  warp_row_stat(a, scale, sh.wstat[row][warp]);
+}
+
+// Consumer warps: level 1 of the draw from the ring (stage = 16 segments of the target row in the first half of a
+// slot and, if use_q, the same 16 of the draft row in the second half).
+template <typename T>
+__device__ __forceinline__ void consume_segment_sums(const unsigned char* ring, Shared& sh,
+                                                     Pipe<Ring<T>::kDepth>& pp, int V, float scale, const RowStats& st, const RowStats& sd, bool use_q,
+                                                     const ClusterCtx& cx, float* seg_sums) {
+  using R = Ring<T>;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int nloc = cx.seg_hi - cx.seg_lo;
+  const int nst = (nloc + kCons - 1) / kCons;
+  for (int k = 0; k < nst; ++k, pp.step()) {
+    er::mbar_wait(&sh.full[pp.slot], pp.phase);
+    const unsigned char* stage = ring + (size_t)pp.slot * R::kStageBytes;
+    const int sg = k * kCons + warp;
+    if (sg < nloc) {
+      const int v0 = (cx.seg_lo + sg) * kSeg + lane * kPerThread;
+      float s = 0.f;
+      if (v0 < V) {
+        const size_t o = (size_t)warp * R::kSegBytes + (size_t)lane * kPerThread * sizeof(T);
+        typename Load8<T>::Raw rp = *reinterpret_cast<const typename Load8<T>::Raw*>(stage + o), rq = rp;
+        clip_tail(rp, v0, V, kNegInf);
+        if (use_q) {
+          rq = *reinterpret_cast<const typename Load8<T>::Raw*>(stage + R::kStageBytes / 2 + o);
+          clip_tail(rq, v0, V, kNegInf);
+        }
+        float w[8];
+        weights8_raw<T, true>(rp, rq, scale, st, sd, use_q, w);
+        s = ((w[0] + w[1]) + (w[2] + w[3])) + ((w[4] + w[5]) + (w[6] + w[7]));
+      }
+      s = warp_sum(s);
+      if (lane == 0) seg_sums[sg] = s;
+    }
+    __syncwarp();
+    if (lane == 0) er::mbar_arrive(&sh.empty[pp.slot]);
+  }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kRingThreads, 1)
+spec_verify_ring_kernel(const T* __restrict__ target, const T* __restrict__ draft, float scale,
+                        const int32_t* __restrict__ draft_tokens, const float* __restrict__ u_accept,
+                        const float* __restrict__ u_sample, int gamma, int V, int32_t* __restrict__ accept_count,
+                        int32_t* __restrict__ out_tokens) {
+  using R = Ring<T>;
+  extern __shared__ __align__(128) unsigned char dyn[];
+  unsigned char* ring = dyn;
+  float* seg_sums = reinterpret_cast<float*>(dyn + kRingBytes);
+  __shared__ Shared sh;
+  cg::cluster_group cluster = cg::this_cluster();
+  ClusterCtx cx;
+  cx.size = (int)cluster.num_blocks();
+  cx.rank = (int)cluster.block_rank();
+  cx.xpar = 0;
+  cx.started = false;
+  if (cx.size > 1) asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory");   // "I have started"
+  const int nseg = (V + kSeg - 1) / kSeg;
+  cx.seg_lo = (int)(((long long)nseg * cx.rank) / cx.size);
+  cx.seg_hi = (int)(((long long)nseg * (cx.rank + 1)) / cx.size);
+  const int b = blockIdx.x / cx.size, tid = threadIdx.x, warp = tid >> 5;
+  const T* tgt = target + (size_t)b * (gamma + 1) * V;
+  const T* drf = draft + (size_t)b * gamma * V;
+  const int32_t* xs = draft_tokens + (size_t)b * gamma;
+  if (tid == 0) {
+    for (int i = 0; i < R::kDepth; ++i) {
+      er::mbar_init(&sh.full[i], 1);
+      er::mbar_init(&sh.empty[i], kCons);
+    }
+    er::mbar_fence_init();
+  }
+  __syncthreads();
+
+  // ---- the sweep: rows t_0, d_0, t_1, d_1, ..., t_gamma ----
+  const int nrows = 2 * gamma + 1;
+  Pipe<R::kDepth> pp;     // the producer lane's, or this consumer warp's
+  if (warp == kCons) {
+    if ((tid & 31) == 0)
+      for (int row = 0; row < nrows; ++row)
+        produce_rows<T>(ring, sh, pp, (row & 1) ? drf + (size_t)(row >> 1) * V : tgt + (size_t)(row >> 1) * V,
+                        (const T*)nullptr, V, cx, kStageSegs);
+  } else {
+    if (tid < gamma) {         // everything the accept tests read, fetched while the ring fills
+      const int x = min(max(xs[tid], 0), V - 1);
+      sh.px[tid] = Load8<T>::one(tgt + (size_t)tid * V, x);
+      sh.qx[tid] = Load8<T>::one(drf + (size_t)tid * V, x);
+      sh.ua[tid] = u_accept[(size_t)b * gamma + tid];
+    }
+    for (int row = 0; row < nrows; ++row) consume_row_stats<T>(ring, sh, pp, row, V, scale, cx);
+  }
+  combine_stats(gamma, kCons, scale, sh, cx);
+  const int n = accept_prefix<true>(gamma, scale, sh);
+  const float4 v = sh.stat[n];
+  const RowStats st = row_stats_of(v.x, v.y, scale), sd = (n < gamma) ? row_stats_of(v.z, v.w, scale) : RowStats{0.f};
+  const T* trow = tgt + (size_t)n * V;
+  const T* drow = (n < gamma) ? drf + (size_t)n * V : nullptr;
+  const float r = u_sample[b];
+  const bool vec = true;
+  int tok = -1;
+  for (int pass = 0; pass < 2 && tok == -1; ++pass) {   // pass 1 only if there is no residual mass: p itself
+    const bool use_q = (pass == 0) && n < gamma;
+    if (pass == 1 && n == gamma) break;
+    if (warp == kCons) {
+      if ((tid & 31) == 0) produce_rows<T>(ring, sh, pp, trow, use_q ? drow : (const T*)nullptr, V, cx, kCons);
+    } else {
+      consume_segment_sums<T>(ring, sh, pp, V, scale, st, sd, use_q, cx, seg_sums);
+    }
+    __syncthreads();
+    tok = draw_finish<T, true>(trow, use_q ? drow : nullptr, V, vec, scale, st, sd, use_q, r, sh, cx, seg_sums);
+  }
+  write_outputs(tok, n, b, gamma, V, xs, cx, accept_count, out_tokens);
 }
 
 template <typename T, bool kLogits>
@@ -565,10 +890,41 @@ int launch_verify(int cluster_size, size_t smem, cudaStream_t s, const T* target
   return ER_OK;
 }
 
+template <typename T>
+int launch_verify_ring(int cluster_size, size_t seg_bytes, cudaStream_t s, const T* target, const T* draft,
+                       float scale, const int32_t* draft_tokens, const float* u_accept, const float* u_sample, int B,
+                       int gamma, int V, int32_t* accept_count, int32_t* out_tokens) {
+  static bool attr_set[er::kMaxDevices];   // the opt-in to > 48 KB of dynamic shared memory is per device
+  const int dev = er::current_device();
+  const size_t smem = (size_t)kRingBytes + seg_bytes;
+  if (dev < 0 || dev >= er::kMaxDevices || !attr_set[dev]) {
+    ER_CUDA_TRY(cudaFuncSetAttribute(spec_verify_ring_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                     kRingBytes + (kMaxV / kSeg) * (int)sizeof(float)));
+    if (dev >= 0 && dev < er::kMaxDevices) attr_set[dev] = true;
+  }
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)(B * cluster_size));
+  cfg.blockDim = dim3(kRingThreads);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = s;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)cluster_size;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  ER_CUDA_TRY(cudaLaunchKernelEx(&cfg, spec_verify_ring_kernel<T>, target, draft, scale, draft_tokens, u_accept,
+                                 u_sample, gamma, V, accept_count, out_tokens));
+  return ER_OK;
+}
+
 #ifdef ER_DEV
-int g_force_cluster = 0;   // development library only (er_dev.h): 0 = automatic
+int g_force_cluster = 0;          // development library only (er_dev.h): 0 = automatic
+int g_force_register_path = 0;    // 1 = never the ring kernel
 #else
 constexpr int g_force_cluster = 0;
+constexpr int g_force_register_path = 0;
 #endif
 
 // CTAs that can be resident at once when launched in clusters of c (one 1024-thread CTA per SM; clusters of 4 / 8
@@ -620,6 +976,10 @@ int pick_cluster(int B, int nseg) {
 
 #ifdef ER_DEV
 extern "C" int er_dev_verify_cluster(int cluster) {
+  if (cluster >= 16 && cluster <= 17) {   // 16 / 17: shared-memory ring kernel allowed / never used
+    g_force_register_path = cluster - 16;
+    return ER_OK;
+  }
   if (cluster != 0 && cluster != 1 && cluster != 2 && cluster != 4 && cluster != 8) return ER_ERR_SHAPE;
   g_force_cluster = cluster;
   return ER_OK;
@@ -645,8 +1005,17 @@ extern "C" int er_spec_verify(const void* target, const void* draft, int in_dtyp
   const size_t smem = (size_t)((nseg + cluster - 1) / cluster) * sizeof(float);   // one sum per local segment
   const float scale = (float)(1.4426950408889634 / (double)temperature);
   cudaStream_t s = (cudaStream_t)stream;
+  const size_t elem = in_dtype == ER_BF16 ? 2 : 4;
+  const bool ring = inputs_are_logits && ((size_t)V * elem) % 16 == 0 && !g_force_register_path;
   int rc;
-  if (in_dtype == ER_F32 && !inputs_are_logits) {
+  if (ring && in_dtype == ER_BF16) {
+    rc = launch_verify_ring<__nv_bfloat16>(cluster, smem, s, (const __nv_bfloat16*)target, (const __nv_bfloat16*)draft,
+                                           scale, draft_tokens, u_accept, u_sample, B, gamma, V, accept_count,
+                                           out_tokens);
+  } else if (ring) {
+    rc = launch_verify_ring<float>(cluster, smem, s, (const float*)target, (const float*)draft, scale, draft_tokens,
+                                   u_accept, u_sample, B, gamma, V, accept_count, out_tokens);
+  } else if (in_dtype == ER_F32 && !inputs_are_logits) {
     rc = launch_verify<float, false>(cluster, smem, s, (const float*)target, (const float*)draft, scale, draft_tokens,
                                      u_accept, u_sample, B, gamma, V, accept_count, out_tokens);
   } else if (in_dtype == ER_F32) {

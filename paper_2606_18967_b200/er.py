@@ -112,6 +112,7 @@ def dev_library():
         for key, value in ((1, 0), (3, 1), (4, 1), (5, 1), (6, 1), (7, 1)):
             lib.er_dev_gemm_tuning(key, value)
         lib.er_dev_verify_cluster(0)
+        lib.er_dev_verify_cluster(16)
         _lib = prev
 
 

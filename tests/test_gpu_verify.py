@@ -66,7 +66,7 @@ def test_q_equals_p_accepts_everything():
     assert np.all(acc == gamma) and np.all(out[:, gamma] >= 0)
 
 
-@pytest.mark.parametrize("V", [1, 7, 255, 8192, 8193, 20011])
+@pytest.mark.parametrize("V", [1, 7, 255, 8192, 8193, 8200, 20011, 20012])
 def test_ragged_vocab_sizes_logits_f32(V):
     B, gamma = 5, 3
     lt, ld = I.verify_logits_f32(B, gamma, V, I.seed_of("ragged", V), draft_noise=0.5)
@@ -219,14 +219,32 @@ def test_max_gamma_and_high_acceptance():
     assert acc.max() >= gamma // 2
 
 
+@pytest.mark.parametrize("ring", [16, 17])
 @pytest.mark.parametrize("cluster", [1, 2, 4, 8])
-def test_every_cluster_size_gives_the_same_tokens(cluster):
-    # the per-sequence work may be split over 1-8 CTAs; decisions and accepted prefixes must not depend on the
-    # split (the drawn token may differ only inside the V10 window, which _run_and_check enforces)
+def test_every_cluster_size_gives_the_same_tokens(cluster, ring):
+    # the per-sequence work may be split over 1-8 CTAs, and the rows may come through the shared-memory ring (16)
+    # or through registers (17); decisions and accepted prefixes must not depend on either (the drawn token may
+    # differ only inside the V10 window, which _run_and_check enforces)
     B, gamma, V = 6, 4, 152064
     lt, ld = I.verify_logits_f32(B, gamma, V, 911, draft_noise=0.5)
     toks = I.sample_draft_tokens(_softmax(ld), 912)
     ua, us = I.uniforms((B, gamma), 913), I.uniforms((B,), 914)
     with er.dev_library() as lib:
-        assert lib.er_dev_verify_cluster(cluster) == 0
+        assert lib.er_dev_verify_cluster(cluster) == 0 and lib.er_dev_verify_cluster(ring) == 0
         _run_and_check(lt, ld, toks, ua, us, True, torch.float32)
+
+
+@pytest.mark.parametrize("V", [8, 264, 50001, 50008, 65536])
+@pytest.mark.parametrize("ring", [16, 17])
+def test_ragged_vocab_sizes_logits_bf16(V, ring):
+    # bf16 rows that are 16-byte multiples take the ring kernel (unless 17 forces the register path), the others
+    # (V = 50001) the register-path kernel with scalar loads
+    B, gamma = 5, 3
+    lt, ld = I.verify_logits_f32(B, gamma, V, I.seed_of("ragged16", V), draft_noise=0.5)
+    t_b = torch.from_numpy(lt).to(torch.bfloat16).float().numpy()
+    d_b = torch.from_numpy(ld).to(torch.bfloat16).float().numpy()
+    toks = I.sample_draft_tokens(_softmax(d_b), V + 1)
+    ua, us = I.uniforms((B, gamma), V + 2), I.uniforms((B,), V + 3)
+    with er.dev_library() as lib:
+        assert lib.er_dev_verify_cluster(ring) == 0
+        _run_and_check(t_b, d_b, toks, ua, us, True, torch.bfloat16)
