@@ -459,7 +459,9 @@ static LargePlan large_plan(int64_t M, int64_t N, int64_t K, int sms, int force_
   for (int mpad = large_mpad_of(M); mpad >= 32; mpad >>= 1) {
     for (int tp = 1; tp <= 1; ++tp) {
       const long long tiles = (long long)(ntiles / tp) * ((M + mpad - 1) / mpad);
-      const double per_group = fmax(450.0 * tp, fmax(4.0 * mpad * tp, 9.6 * mpad));
+      // X boxes: 4.8 cycles per 128-byte row measured up to MPAD = 128, 5.8 at MPAD = 256 (every SM re-reads all of X
+      // from L2 for every tile: at 256 rows the L2 -> SM traffic of X alone is ~7 TB/s)
+      const double per_group = fmax(450.0 * tp, fmax(4.0 * mpad * tp, (mpad == 256 ? 11.6 : 9.6) * mpad));
       {  // whole tiles
         const int c = (int)(tiles < ctas ? tiles : ctas);
         const double cyc = (double)((tiles + c - 1) / c) * G * per_group + 2000.0;
@@ -477,14 +479,12 @@ static LargePlan large_plan(int64_t M, int64_t N, int64_t K, int sms, int force_
   return best;
 }
 
-// Where the large-batch kernel is preferred over the exact per-group kernel (measured on the 7B / 32B shapes,
-// profiles/r02_gemm.md): from M > 64 on, when it gets whole tiles on at least ~45 % of the SMs AND the reduction is not
-// long (K <= 8192).  On long-K / few-tile shapes (`down`: 28-40 tiles x 148-216 groups) whole tiles leave most of the
-// machine idle and its split-K partial tiles are up to 128 KB each: the exact kernel's stream-K is faster there.
+// Where the large-batch kernel is preferred over the exact per-group kernel: from M > 64 on (measured on the 7B / 32B
+// shapes, profiles/r02_gemm.md section 6).  There the exact kernel needs two to four passes of 64 rows and converts
+// every weight once per pass; up to M = 64 its one pass and its cluster / stream-K partitions are faster.
 bool large_preferred(int64_t M, int64_t N, int64_t K) {
-  if (M <= 64 || K > 8192) return false;
-  const LargePlan pl = large_plan(M, N, K, sm_count(), g_tune.force_ctas);
-  return pl.unit_groups > 1 && (long long)pl.ctas * 100 >= (long long)sm_count() * 45;
+  (void)N; (void)K;
+  return M > 64;
 }
 
 size_t large_workspace_bytes(int64_t M, int64_t N, int64_t K) {

@@ -52,19 +52,23 @@ def test_config0(simt):
     _check(x, qw, sc, simt=simt)
 
 
-@pytest.mark.parametrize("simt", [True, False])
-def test_one_hot_reads_out_dequantised_matrix(simt):
-    # x[m] = e_k: y[m][n] must equal q[n][k] * s[k//128][n] exactly (pins layout, dequant, transpose)
+@pytest.mark.parametrize("simt,rows", [(True, 256), (False, 64), (False, 256)])
+def test_one_hot_reads_out_dequantised_matrix(simt, rows):
+    # x[m] = e_k: y[m][n] must equal the dequantised weight of the kernel that serves this batch size, exactly (pins
+    # layout, dequant, transpose): q[n][k] * s[k//128][n] for M <= 64 (and the SIMT kernel at any M), and that
+    # product rounded to bf16 (RNE) for M > 64, where er.h states that the weights are pre-scaled in bf16
     N, K = 256, 512
     codes = I.random_codes(N, K, 3)          # includes -8
     su = _random_scales(K // 128, N, 4)
     qw, sc = _dev_weights(codes, su)
-    wd = O.dequantize(O.pack_codes(codes), su)      # [N][K] fp64, exact
-    for k0 in range(0, K, 256):
-        x = torch.zeros((256, K), dtype=torch.bfloat16, device=DEV)
-        x[torch.arange(256), k0 + torch.arange(256)] = 1.0
+    wd = O.dequantize(O.pack_codes(codes), su)      # [N][K] fp64, exact (<= 12 significant bits)
+    if rows > 64 and not simt:
+        wd = torch.from_numpy(wd).to(torch.float32).to(torch.bfloat16).to(torch.float64).numpy()
+    for k0 in range(0, K, rows):
+        x = torch.zeros((rows, K), dtype=torch.bfloat16, device=DEV)
+        x[torch.arange(rows), k0 + torch.arange(rows)] = 1.0
         y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32, simt=simt).cpu().numpy().astype(np.float64)
-        assert np.array_equal(y, wd[:, k0:k0 + 256].T)
+        assert np.array_equal(y, wd[:, k0:k0 + rows].T)
 
 
 def test_counting_pattern_layout():
