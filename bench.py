@@ -398,7 +398,8 @@ def model_detail(torch, er, I, dev, mode, peak, gammas=(2, 4, 8), Ms=(256, 128, 
     w4_bytes = W4_BYTES_PER_WEIGHT * n_params
     lm_bytes = 2.0 * V * H
     out = {"refresh_whole_model": refresh, "steps": []}
-    for M in Ms:
+    for M in sorted(Ms):     # ascending: the long tensor-bound steps at M = 256 (T_V: 2304 rows of bf16 GEMMs) pull the SM
+                             # clock down under the power cap for a while; the small-batch rows are timed before them
         h0 = I.activation_bf16(M, H, I.seed_of("model", "h", M), device=dev)
         # the parts of one drafter step, each as its own graph
         t_layers = _graph_time_us(torch, lambda: layers(h0, w4), 1, mode)
