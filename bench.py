@@ -243,6 +243,65 @@ def reference_arm(args):
 # ------------------------------------------------------------------------------------------------------
 # product arm
 # ------------------------------------------------------------------------------------------------------
+def policy_detail(er, I, model):
+    """SURVEY 8(f) f2 on this box, through the C ABI (host scalars): the roofline model of PAPER.md:L111-L115 calibrated
+    (L478-L484) on the T_p / T_q / T_V that model_detail measured, the toggle pi_SD of Eq. 3 per active batch checked
+    against the empirical Eq. 5 speedup, and the shrinking-batch rollout driver (AR, SD throughout, pi_SD).  There is no
+    attention / KV cache on this path: S = 0 and kappa = C_attn = 0 (rho_kappa stays unidentified)."""
+    shape = I.SHAPE_7B
+    n_lin = sum(N * K for _, N, K in shape.linears()) * shape.layers
+    n_head = shape.vocab * shape.hidden
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            F_eff, f_src = float(json.load(f)["bf16_tflops_sustained"]) * 1e12, "MEASURED_PEAKS.json bf16_tflops_sustained"
+    except Exception:
+        F_eff, f_src = 1.4e15, "fallback"
+    start = er.RooflineModel(W_T=2.0 * (n_lin + n_head), W_D=W4_BYTES_PER_WEIGHT * n_lin + 2.0 * n_head,
+                             C_dense=2.0 * (n_lin + n_head), C_attn=0.0, kappa=0.0, F_eff=F_eff, BW_eff=hbm_peak()[0] * 1e9,
+                             rho_kappa=0.0, eta_D=1.0, c_T=0.0, c_D=0.0, c_V=0.0, c_comm=0.0)
+    steps = model["steps"]
+    target = [(s["M"], 0.0, s["T_p_us"] * 1e-6) for s in steps]
+    drafter = [(s["M"], 0.0, s["T_q_us"] * 1e-6) for s in steps]
+    verify = [(s["M"], 0.0, g["gamma"], g["T_V_us"] * 1e-6) for s in steps for g in s["per_gamma"]]
+    fit = er.roofline_calibrate(start, target, drafter, verify)
+    eps = 0.05                                   # PAPER.md:L175
+    import numpy as np
+    per_alpha = {}
+    # alpha = 0.981: PAPER.md:L188 (Table 2, Qwen2.5-7B); 0.802: the acceptance of config 4's synthetic drafter (SURVEY App. B)
+    for alpha in (0.981, 0.802):
+        rows, agree, total = [], 0, 0
+        for s in steps:
+            for g in s["per_gamma"]:
+                tau = er.tau_of_alpha(alpha, g["gamma"])
+                on, pred = er.sd_toggle(fit, s["M"], 0.0, tau, g["gamma"], eps)
+                emp = tau * s["T_p_us"] / (g["gamma"] * s["T_q_us"] + g["T_V_us"])
+                rows.append({"B": s["M"], "gamma": g["gamma"], "predicted_speedup": round(pred, 3),
+                             "empirical_speedup_eq5": round(emp, 3), "pi_sd": on})
+                agree += int((emp >= 1.0 + eps) == bool(on))
+                total += 1
+        sims = {}
+        for n_seq in (128, 2048):                # 128: PAPER.md:L536 (1024 rollouts over 8 DP workers); 2048: beyond the
+            gen = np.random.default_rng(I.seed_of("bench", "rollout", n_seq))   # measured batches, the model extrapolates
+            lengths = (gen.lognormal(6.5, 0.9, size=n_seq).clip(max=8191).astype(int) + 1).tolist()
+            sim = {}
+            for gamma in (5, 7, 9, 11):          # the paper's draft-length set
+                tau = er.tau_of_alpha(alpha, gamma)
+                t = [er.rollout_simulate(fit, lengths, 0.0, gamma, tau, eps, mode) for mode in (0, 1, 2)]
+                sim[str(gamma)] = {"ar_ms": round(t[0][0] * 1e3, 1), "sd_always_ms": round(t[1][0] * 1e3, 1),
+                                   "pi_sd_ms": round(t[2][0] * 1e3, 1), "pi_sd_steps": t[2][1], "pi_sd_ar_steps": t[2][2],
+                                   "pi_sd_reduction_vs_ar": round(1.0 - t[2][0] / t[0][0], 4),
+                                   "sd_always_reduction_vs_ar": round(1.0 - t[1][0] / t[0][0], 4)}
+            sims[f"{n_seq}_seqs"] = sim
+        per_alpha[str(alpha)] = {"toggle": rows, "toggle_agrees_with_eq5": f"{agree}/{total}", "rollout_driver": sims}
+    return {"fitted": {"F_eff_tflops": round(F_eff / 1e12, 1), "F_eff_source": f_src,
+                       "BW_eff_gbs": round(fit.BW_eff / 1e9, 1), "eta_D": round(fit.eta_D, 4),
+                       "c_T_us_per_seq": round(fit.c_T * 1e6, 3), "c_D_us_per_seq": round(fit.c_D * 1e6, 3),
+                       "c_V_us_per_seq": round(fit.c_V * 1e6, 3), "W_D_over_W_T": round(start.W_D / start.W_T, 4)},
+            "eps": eps, "per_alpha": per_alpha,
+            "note": "S = 0 (no attention / KV cache on this path); glue stand-ins are inside T_p / T_q / T_V"}
+
+
+
 def _graph_time_us(torch, body, launches, mode, reps=3):
     """Average microseconds per launch of `body` (which enqueues `launches` kernels on the current stream): captured
     once in a CUDA graph on a side stream, replayed `reps` + 1 times, best replay, CUDA events on that stream."""
@@ -605,6 +664,7 @@ def product_arm(args):
         del src, qw, sc                      # the whole-model pass needs the memory of the step's layer copies
         torch.cuda.empty_cache()
         model = model_detail(torch, er, I, dev, mode, peak)
+        model["sd_policy"] = policy_detail(er, I, model)
     torch.cuda.synchronize()
 
     stats = torch.cat([blk_ms, det.flatten(), torch.tensor([step_ms], dtype=torch.float64)])

@@ -203,6 +203,57 @@ int er_spec_verify_host(const void* target_host, const void* draft_host, int in_
                         const float* u_sample_host, int32_t B, int32_t gamma, int32_t V, int32_t* accept_count_host,
                         int32_t* out_tokens_host, void* arena, size_t arena_bytes, void* stream);
 
+/* ---- SD toggle, draft length and calibration ---------------------------------------------------
+ * Scalar HOST logic of the paper's method around the three kernels: every pointer below is a HOST pointer, nothing
+ * touches a device, the calls work without a GPU.  Units are SI (bytes, flop, seconds).
+ *   er_roofline_model   PAPER.md:L111 (M_T, M_D, C), L455-L469 (parameter details), L473 Eq. 4 (c_comm; 0 for TP = 1):
+ *     static, from the architecture:  W_T, W_D weight bytes of target and W4 drafter; C_dense flop per token; C_attn
+ *       flop per token and per token of context; kappa theoretical KV bytes per token of context
+ *     calibrated: F_eff (stage 1, flop/s), BW_eff (bytes/s), rho_kappa, eta_D, c_T, c_D, c_V (seconds per sequence)
+ *   er_tau_of_alpha       tau = (1 - alpha^(gamma+1)) / (1 - alpha); gamma + 1 at alpha = 1
+ *   er_alpha_of_tau       its inverse on [0, 1], clamped: 0 for tau <= 1, 1 for tau >= gamma + 1
+ *   er_roofline_times     T_p = max{M_T, C} + c_T B, T_q = max{M_D, C} + c_D B, T_V = max{M_T, (gamma+1) C} + c_V B,
+ *                         each + c_comm
+ *   er_sd_toggle          pi_SD of Eq. 3: *on = 1 iff tau T_p / (gamma T_q + T_V) >= 1 + eps; the
+ *                         predicted speedup goes to *speedup if that is not NULL.  (Stickiness -- "once activated, SD
+ *                         remains enabled until the end of the rollout", L122 -- is the caller's one flag.)
+ *   er_gamma_next         Alg. 1 lines 11-12: Gamma[0..n) ascending, gamma_t a member; tau_hist the
+ *                         block efficiencies recorded so far, oldest first; returns in *gamma_out next_Gamma(gamma_t) if
+ *                         the minimum of the last P is >= 1 + gamma_t alpha_up (and gamma_t < gamma_high), prev_Gamma if
+ *                         the maximum of the last P is <= 1 + gamma_t alpha_down (and gamma_t > gamma_low), else gamma_t
+ *                         (also when fewer than P values are recorded).  Paper's setting: {5,7,9,11}, 0.94, 0.85, P = 2.
+ *   er_roofline_calibrate PAPER.md:L478-L484, steps 2-3 (F_eff and the static terms come in through *model): the target
+ *                         sweep (B, S, T_p) fits BW_eff, rho_kappa, c_T; then, with those fixed, the drafter sweep
+ *                         (B, S, T_q) fits eta_D, c_D and the verification sweep (B, S, gamma, T_V) fits c_V.  Ordinary
+ *                         least squares on seconds; a sample counts as memory- or compute-bound by the current estimate
+ *                         and classification and fit are iterated to a fixed point, starting from the values in *model
+ *                         (readings P1-P2).  Arrays are parallel, n_* entries each; a sweep with n = 0 leaves
+ *                         its parameters unchanged.  *model is updated in place.
+ *   er_rollout_simulate   measurement driver (reading P5, not part of the paper): a batch of `n` responses of
+ *                         lengths[i] tokens decoded in lockstep, B = #{lengths > position}, S = S0 + position; an AR step
+ *                         costs T_p and advances 1 token, an SD block costs gamma T_q + T_V and advances tau tokens.
+ *                         mode 0: AR only, 1: SD throughout, 2: pi_SD decides, sticky.  Outputs: seconds, steps, and
+ *                         the steps decoded autoregressively.
+ * Errors: ER_ERR_NULL, ER_ERR_SHAPE (gamma < 1, n < 0, P < 1, gamma_t not in Gamma, Gamma not ascending, a
+ * non-positive F_eff / BW_eff, mode outside 0..2). */
+typedef struct {
+  double W_T, W_D, C_dense, C_attn, kappa;
+  double F_eff, BW_eff, rho_kappa, eta_D, c_T, c_D, c_V, c_comm;
+} er_roofline_model;
+int er_tau_of_alpha(double alpha, int32_t gamma, double* tau_out);
+int er_alpha_of_tau(double tau, int32_t gamma, double* alpha_out);
+int er_roofline_times(const er_roofline_model* model, double B, double S, int32_t gamma, double* T_p, double* T_q,
+                      double* T_V);
+int er_sd_toggle(const er_roofline_model* model, double B, double S, double tau, int32_t gamma, double eps, int32_t* on,
+                 double* speedup);
+int er_gamma_next(const int32_t* Gamma, int32_t n, int32_t gamma_t, const double* tau_hist, int32_t n_hist, int32_t P,
+                  double alpha_up, double alpha_down, int32_t* gamma_out);
+int er_roofline_calibrate(er_roofline_model* model, const double* tB, const double* tS, const double* tT, int32_t n_target,
+                          const double* dB, const double* dS, const double* dT, int32_t n_drafter, const double* vB,
+                          const double* vS, const int32_t* vgamma, const double* vT, int32_t n_verify);
+int er_rollout_simulate(const er_roofline_model* model, const double* lengths, int32_t n, double S0, int32_t gamma,
+                        double tau, double eps, int32_t mode, double* seconds, int64_t* steps, int64_t* ar_steps);
+
 #ifdef __cplusplus
 }
 #endif

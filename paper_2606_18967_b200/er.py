@@ -26,6 +26,12 @@ class LinearDesc(ctypes.Structure):
                 ("qweight", ctypes.c_void_p), ("scales", ctypes.c_void_p)]
 
 
+class RooflineModel(ctypes.Structure):
+    """er_roofline_model of include/er.h (SI units)."""
+    _fields_ = [(n, ctypes.c_double) for n in ("W_T", "W_D", "C_dense", "C_attn", "kappa", "F_eff", "BW_eff",
+                                               "rho_kappa", "eta_D", "c_T", "c_D", "c_V", "c_comm")]
+
+
 class ErError(RuntimeError):
     def __init__(self, status: int, where: str):
         lib = load()
@@ -79,6 +85,16 @@ def _bind(lib: ctypes.CDLL) -> ctypes.CDLL:
     lib.er_spec_verify_host.restype = ctypes.c_int
     lib.er_spec_verify_host.argtypes = [vp, vp, ctypes.c_int, ctypes.c_int, f32, vp, vp, vp, i32, i32, i32, vp, vp, vp,
                                         sz, vp]
+    f64, pd, pm = ctypes.c_double, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(RooflineModel)
+    pi32, pi64 = ctypes.POINTER(i32), ctypes.POINTER(i64)
+    for name, args in (("er_tau_of_alpha", [f64, i32, pd]), ("er_alpha_of_tau", [f64, i32, pd]),
+                       ("er_roofline_times", [pm, f64, f64, i32, pd, pd, pd]),
+                       ("er_sd_toggle", [pm, f64, f64, f64, i32, f64, pi32, pd]),
+                       ("er_gamma_next", [pi32, i32, i32, pd, i32, i32, f64, f64, pi32]),
+                       ("er_roofline_calibrate", [pm, pd, pd, pd, i32, pd, pd, pd, i32, pd, pd, pi32, pd, i32]),
+                       ("er_rollout_simulate", [pm, pd, i32, f64, i32, f64, f64, i32, pd, pi64, pi64])):
+        getattr(lib, name).restype = ctypes.c_int
+        getattr(lib, name).argtypes = args
     if lib.er_abi_version() != 1:
         raise RuntimeError("liber_b200.so ABI version mismatch")
     return lib
@@ -304,3 +320,64 @@ def spec_verify_host(target: torch.Tensor, draft: torch.Tensor, draft_tokens: to
                                       out_tokens.data_ptr(), arena.data_ptr(), arena.numel(), _stream(arena)),
            "er_spec_verify_host")
     return accept_count, out_tokens
+
+
+# ---- SD toggle, draft length, calibration (include/er.h): host scalars in, host scalars out ----------
+def _darr(xs):
+    xs = [float(x) for x in xs]
+    return (ctypes.c_double * len(xs))(*xs), len(xs)
+
+
+def tau_of_alpha(alpha: float, gamma: int) -> float:
+    out = ctypes.c_double()
+    _check(load().er_tau_of_alpha(alpha, gamma, ctypes.byref(out)), "er_tau_of_alpha")
+    return out.value
+
+
+def alpha_of_tau(tau: float, gamma: int) -> float:
+    out = ctypes.c_double()
+    _check(load().er_alpha_of_tau(tau, gamma, ctypes.byref(out)), "er_alpha_of_tau")
+    return out.value
+
+
+def roofline_times(model: RooflineModel, B: float, S: float, gamma: int):
+    tp, tq, tv = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+    _check(load().er_roofline_times(ctypes.byref(model), B, S, gamma, ctypes.byref(tp), ctypes.byref(tq),
+                                    ctypes.byref(tv)), "er_roofline_times")
+    return tp.value, tq.value, tv.value
+
+
+def sd_toggle(model: RooflineModel, B: float, S: float, tau: float, gamma: int, eps: float):
+    on, s = ctypes.c_int32(), ctypes.c_double()
+    _check(load().er_sd_toggle(ctypes.byref(model), B, S, tau, gamma, eps, ctypes.byref(on), ctypes.byref(s)),
+           "er_sd_toggle")
+    return on.value, s.value
+
+
+def gamma_next(Gamma, gamma_t: int, tau_hist, P: int, alpha_up: float, alpha_down: float) -> int:
+    G = (ctypes.c_int32 * len(Gamma))(*[int(g) for g in Gamma])
+    h, nh = _darr(tau_hist)
+    out = ctypes.c_int32()
+    _check(load().er_gamma_next(G, len(Gamma), gamma_t, h, nh, P, alpha_up, alpha_down, ctypes.byref(out)),
+           "er_gamma_next")
+    return out.value
+
+
+def roofline_calibrate(model: RooflineModel, target, drafter, verify) -> RooflineModel:
+    """target rows (B, S, T_p), drafter rows (B, S, T_q), verify rows (B, S, gamma, T_V); returns the fitted copy."""
+    out = RooflineModel.from_buffer_copy(model)
+    tb, nt = _darr([r[0] for r in target]); ts, _ = _darr([r[1] for r in target]); tt, _ = _darr([r[2] for r in target])
+    db, nd = _darr([r[0] for r in drafter]); ds, _ = _darr([r[1] for r in drafter]); dt, _ = _darr([r[2] for r in drafter])
+    vb, nv = _darr([r[0] for r in verify]); vs, _ = _darr([r[1] for r in verify]); vt, _ = _darr([r[3] for r in verify])
+    vg = (ctypes.c_int32 * nv)(*[int(r[2]) for r in verify])
+    _check(load().er_roofline_calibrate(ctypes.byref(out), tb, ts, tt, nt, db, ds, dt, nd, vb, vs, vg, vt, nv),
+           "er_roofline_calibrate")
+    return out
+
+
+def rollout_simulate(model: RooflineModel, lengths, S0: float, gamma: int, tau: float, eps: float, mode: int):
+    L, n = _darr(lengths)
+    sec, steps, ar = ctypes.c_double(), ctypes.c_int64(), ctypes.c_int64()
+    _check(load().er_rollout_simulate(ctypes.byref(model), L, n, S0, gamma, tau, eps, mode, ctypes.byref(sec),
+                                      ctypes.byref(steps), ctypes.byref(ar)), "er_rollout_simulate")
+    return sec.value, steps.value, ar.value
