@@ -23,6 +23,8 @@
  *     not sm_100 the compute calls return ER_ERR_ARCH.
  *   - Determinism: identical inputs give bit-identical outputs (fixed split-K reduction order, no
  *     floating-point atomics).
+ *   - Host-side state is limited to per-device caches of idempotent values (SM count, occupancy answers, "shared-memory
+ *     opt-in done"); the calls may be made from several host threads and on several devices of one process.
  *
  * Data layouts:
  *   W        bf16 [N][K], row-major, K contiguous, row stride ldw elements (torch nn.Linear.weight)
@@ -167,7 +169,11 @@ int er_bf16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, co
  *   out_tokens   int32 [B][gamma+1] out: x_1..x_n, then the token drawn at position n+1 by inverse CDF
  *            (vocab order, token = min{v : C(v) > u_sample * R}) from w = max(0, p_{n+1} - q_{n+1})
  *            (n < gamma; w = p_{n+1} if that residual is identically 0) or w = p_{gamma+1} (n == gamma),
- *            then -1 padding. */
+ *            then -1 padding.
+ *   Logits may be -inf (masked tokens: probability 0); a row needs at least one finite logit.  Arithmetic for logits:
+ *   p(v) = 2^((l_v - m) * log2(e) / temperature) / sum, fp32, with ex2.approx (relative error 2^-22) and m a logit of the
+ *   row within 32 * temperature / log2(e) of its maximum (a lazily raised reference: no term exceeds 2^32); the accept
+ *   test and the residual use the same (m, sum).  One launch, one thread-block cluster per sequence. */
 int er_spec_verify(const void* target, const void* draft, int in_dtype, int inputs_are_logits,
                    float temperature, const int32_t* draft_tokens, const float* u_accept,
                    const float* u_sample, int32_t B, int32_t gamma, int32_t V,

@@ -833,17 +833,19 @@ spec_verify_ring_kernel(const T* __restrict__ target, const T* __restrict__ draf
   const int nrows = 2 * gamma + 1;
   Pipe<R::kDepth> pp;     // the producer lane's, or this consumer warp's
   if (warp == kCons) {
-    if ((tid & 31) == 0)
+    const int lane = tid & 31;
+    if (lane == 0) {
       for (int row = 0; row < nrows; ++row)
         produce_rows<T>(ring, sh, pp, (row & 1) ? drf + (size_t)(row >> 1) * V : tgt + (size_t)(row >> 1) * V,
                         (const T*)nullptr, V, cx, kStageSegs);
-  } else {
-    if (tid < gamma) {         // everything the accept tests read, fetched while the ring fills
-      const int x = min(max(xs[tid], 0), V - 1);
-      sh.px[tid] = Load8<T>::one(tgt + (size_t)tid * V, x);
-      sh.qx[tid] = Load8<T>::one(drf + (size_t)tid * V, x);
-      sh.ua[tid] = u_accept[(size_t)b * gamma + tid];
+    } else if (lane <= gamma) {   // everything the accept tests read, fetched by the producer warp's idle lanes (a
+      const int k = lane - 1;     // consumer warp waiting for these two round trips would hold back the whole ring)
+      const int x = min(max(xs[k], 0), V - 1);
+      sh.px[k] = Load8<T>::one(tgt + (size_t)k * V, x);
+      sh.qx[k] = Load8<T>::one(drf + (size_t)k * V, x);
+      sh.ua[k] = u_accept[(size_t)b * gamma + k];
     }
+  } else {
     for (int row = 0; row < nrows; ++row) consume_row_stats<T>(ring, sh, pp, row, V, scale, cx);
   }
   combine_stats(gamma, kCons, scale, sh, cx);
