@@ -155,7 +155,7 @@ def test_config4_full_batch_64(gamma):
 
 
 def test_config2_maximum_batch_256_gamma_8():
-    # config 2's largest verify (B = M = 256, gamma = 8): 2048 CTAs in clusters of 8, several residency waves; every
+    # config 2's largest verify (B = M = 256, gamma = 8): 1024 CTAs in clusters of 4, seven residency waves; every
     # sequence's structural properties + the oracle on a seeded quarter of the sequences
     B, gamma, V = 256, 8, 152064
     tgt, drf, toks, ua, us = _device_workload(B, gamma, V, "cfg2max")
@@ -248,3 +248,43 @@ def test_ragged_vocab_sizes_logits_bf16(V, ring):
     with er.dev_library() as lib:
         assert lib.er_dev_verify_cluster(ring) == 0
         _run_and_check(t_b, d_b, toks, ua, us, True, torch.bfloat16)
+
+
+@pytest.mark.parametrize("cluster", [0, 1])
+def test_maximum_vocabulary(cluster):
+    # V = 2^20, the largest the call accepts: 4096 segments; with one CTA per sequence (cluster 1) the segment-sum
+    # array and the fp64 blocked prefix are at their largest
+    B, gamma, V = 2, 2, 1 << 20
+    lt, ld = I.verify_logits_f32(B, gamma, V, 31337, draft_noise=0.5)
+    t_b = torch.from_numpy(lt).to(torch.bfloat16).float().numpy()
+    d_b = torch.from_numpy(ld).to(torch.bfloat16).float().numpy()
+    toks = I.sample_draft_tokens(_softmax(d_b), 31338)
+    ua, us = I.uniforms((B, gamma), 31339), I.uniforms((B,), 31340)
+    with er.dev_library() as lib:
+        assert lib.er_dev_verify_cluster(cluster) == 0
+        _run_and_check(t_b, d_b, toks, ua, us, True, torch.bfloat16)
+    lib = er.load()
+    z = torch.zeros(16, device=DEV)
+    assert lib.er_spec_verify(z.data_ptr(), z.data_ptr(), 0, 1, 1.0, z.data_ptr(), z.data_ptr(), z.data_ptr(), 1, 2,
+                              (1 << 20) + 8, z.data_ptr(), z.data_ptr(), None) == 2       # ER_ERR_SHAPE
+
+
+@pytest.mark.parametrize("dtype", [torch.float32, torch.bfloat16])
+@pytest.mark.parametrize("ring", [16, 17])
+def test_rising_logits_raise_the_softmax_reference_many_times(dtype, ring):
+    # logits that climb along the vocabulary by far more than the 32-bit margin of the lazily raised reference (range
+    # 600 / T = 0.5 -> ~1700 binades): every lane has to re-reference its sums again and again, in both kernels; the
+    # statistics must still match the fp64 oracle (accept counts exact, token by rule V10)
+    B, gamma, V = 4, 3, 40000
+    rng = np.random.default_rng(99)
+    ramp = np.linspace(-300.0, 300.0, V, dtype=np.float32)
+    lt = (ramp[None, None, :] + rng.standard_normal((B, gamma + 1, V)).astype(np.float32)).astype(np.float32)
+    ld = (lt[:, :gamma] + 0.3 * rng.standard_normal((B, gamma, V)).astype(np.float32)).astype(np.float32)
+    lt[1], ld[1] = lt[1, :, ::-1].copy(), ld[1, :, ::-1].copy()          # one sequence falls instead of climbing
+    t_h = torch.from_numpy(lt).to(dtype).float().numpy()
+    d_h = torch.from_numpy(ld).to(dtype).float().numpy()
+    toks = I.sample_draft_tokens(O.softmax64(d_h, 0.5).astype(np.float32), 100)
+    ua, us = I.uniforms((B, gamma), 101), I.uniforms((B,), 102)
+    with er.dev_library() as lib:
+        assert lib.er_dev_verify_cluster(ring) == 0
+        _run_and_check(t_h, d_h, toks, ua, us, True, dtype, temperature=0.5)
