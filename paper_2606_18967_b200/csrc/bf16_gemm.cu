@@ -233,30 +233,45 @@ bf16_gemm_kernel(const __grid_constant__ CUtensorMap map_w, const __grid_constan
       for (int k = 0; k < 2; ++k) {
         if (pend_tile[k] < 0 || last_flag[k] == 0) continue;
         const int tile = pend_tile[k];
-        const int n = (tile % p.ntiles) * kTileN + row, m_base = (tile / p.ntiles) * MPAD;
+        const int n0 = (tile % p.ntiles) * kTileN, m_base = (tile / p.ntiles) * MPAD;
+        // a partial tile is [MPAD][128] fp32: the 128 threads walk it as float4 (thread t: batch row 4 i + t / 32, four
+        // consecutive n from (t % 32) * 4), kI rows of loads in flight per partial, partials added in ascending CTA order
+        const int t = threadIdx.x, col4 = (t & 31) * 4;
+        constexpr int kI = 8;
 #pragma unroll 1
-        for (int c0 = 0; c0 < MPAD; c0 += 8) {
-          if (m_base + c0 >= p.M) break;
-          float acc[8];
+        for (int i0 = 0; i0 < MPAD / 4; i0 += kI) {
+          if (m_base + 4 * i0 >= p.M) break;
+          float4 acc[kI];
 #pragma unroll
-          for (int j = 0; j < 8; ++j) acc[j] = 0.f;
+          for (int i = 0; i < kI; ++i) acc[i] = make_float4(0.f, 0.f, 0.f, 0.f);
           for (int c = c_lo[k]; c <= c_hi[k]; ++c) {
             // CTA c's piece of this tile is its first segment iff its range starts inside the tile
             const int cb = range_begin(p.uq, p.ur, p.split, c) * ug;
             const int which = (cb >= tile * p.G) ? 0 : 1;
             const float* src = p.partials + ((size_t)c * 2 + which) * (MPAD * kTileN);
-            float t[8];
+            float4 v[kI];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) t[j] = (m_base + c0 + j < p.M) ? __ldcg(src + (c0 + j) * kTileN + row) : 0.f;
+            for (int i = 0; i < kI; ++i) {
+              const int m = 4 * (i0 + i) + (t >> 5);
+              v[i] = (i0 + i < MPAD / 4 && m_base + m < p.M) ? __ldcg(reinterpret_cast<const float4*>(src + m * kTileN + col4))
+                                                            : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
 #pragma unroll
-            for (int j = 0; j < 8; ++j) acc[j] += t[j];
+            for (int i = 0; i < kI; ++i) { acc[i].x += v[i].x; acc[i].y += v[i].y; acc[i].z += v[i].z; acc[i].w += v[i].w; }
           }
 #pragma unroll
-          for (int j = 0; j < 8; ++j) {
-            const int m = m_base + c0 + j;
-            if (m < p.M) {
-              if (p.y_f32) reinterpret_cast<float*>(p.y)[(size_t)m * p.ldy + n] = acc[j];
-              else reinterpret_cast<__nv_bfloat16*>(p.y)[(size_t)m * p.ldy + n] = __float2bfloat16_rn(acc[j]);
+          for (int i = 0; i < kI; ++i) {
+            const int m = m_base + 4 * (i0 + i) + (t >> 5);
+            if (i0 + i < MPAD / 4 && m < p.M) {
+              const size_t o = (size_t)m * p.ldy + n0 + col4;
+              if (p.y_f32) {
+                float* y = reinterpret_cast<float*>(p.y) + o;      // ldy is not necessarily a multiple of 4: scalar stores
+                y[0] = acc[i].x; y[1] = acc[i].y; y[2] = acc[i].z; y[3] = acc[i].w;
+              } else {
+                __nv_bfloat16* y = reinterpret_cast<__nv_bfloat16*>(p.y) + o;
+                y[0] = __float2bfloat16_rn(acc[i].x); y[1] = __float2bfloat16_rn(acc[i].y);
+                y[2] = __float2bfloat16_rn(acc[i].z); y[3] = __float2bfloat16_rn(acc[i].w);
+              }
             }
           }
         }
@@ -298,6 +313,43 @@ int launch(const CUtensorMap& mw, const CUtensorMap& mx, const GemmParams& gp, i
   return ER_OK;
 }
 
+// Plan: the padded batch MPAD (the N of the MMA) may be SMALLER than M -- the batch is then cut into chunks, every (chunk,
+// 128-row weight tile) is a tile of its own, and a tile's weights are read once per chunk (from L2 after the first).
+// That buys whole tiles for most SMs on the small linears, where stream-K would leave partial tiles of MPAD x 128 fp32
+// for the last CTA of a tile to add up (128 threads: ~12 bytes per clock).  Costs per 128-k group in SM cycles, fitted
+// to the lm_head timings (profiles/r02_gemm.md section 7): 800 + 4.9 MPAD with the weights in L2 (the X box is re-read
+// for every tile), 1440 when the weights stream from HBM at the measured peak.
+struct BPlan { int mpad, whole, ctas; double cycles; };
+BPlan bf16_plan(int64_t M, int64_t N, int64_t K) {
+  const int sms = er::sm_count();
+  const int cap = (er::g_tune.force_ctas > 0 && er::g_tune.force_ctas < sms) ? er::g_tune.force_ctas : sms;
+  const int ntiles = (int)(N / kTileN);
+  const double G128 = (double)K / 128.0;
+  const double hbm = (double)N * (double)K * 2.0 / 22.7 / sms;   // cycles to stream all weights once: 22.7 B / clock / SM
+  BPlan best = {mpad_of(M), 0, 1, 1e300};
+  for (int mpad = mpad_of(M); mpad >= 16; mpad >>= 1) {
+    const long long tiles = (long long)ntiles * ((M + mpad - 1) / mpad);
+    const double per_group = 800.0 + 4.9 * mpad;
+    if (er::g_tune.force_ctas == 0) {   // whole tiles
+      const int c = (int)(tiles < cap ? tiles : cap);
+      const double cyc = fmax((double)((tiles + c - 1) / c) * G128 * per_group, hbm) + 3000.0;
+      if (cyc < best.cycles) best = {mpad, 1, c, cyc};
+    }
+    if (tiles <= ER_GEMM_COUNTER_BYTES / 4) {   // stream-K: units of uk k, partial tiles through the workspace
+      const int uk = uk_of(mpad);
+      const long long upt = K / uk, units = tiles * upt;
+      const int c = (int)(units < cap ? units : cap);
+      const double per_unit = per_group * uk / 128.0;
+      const bool aligned = units % c == 0 && (units / c) % upt == 0;            // every CTA gets whole tiles anyway
+      const double parts = fmin((double)c / (double)tiles + 1.0, (double)c);     // partial tiles the last CTA adds
+      const double cyc = fmax((double)((units + c - 1) / c) * per_unit, hbm) + (aligned ? 0.0 : parts * mpad * 512.0 / 12.0) +
+                         6000.0;
+      if (cyc < best.cycles) best = {mpad, 0, c, cyc};
+    }
+  }
+  return best;
+}
+
 }  // namespace
 
 extern "C" {
@@ -318,21 +370,18 @@ int er_bf16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, co
   if (!er::aligned16(x_bf16) || !er::aligned16(w_bf16) || (ldx_elems % 8) != 0 || (ldw_elems % 8) != 0) return ER_ERR_ALIGN;
   if (!workspace) return ER_ERR_WORKSPACE;
   if (!er::aligned16(workspace)) return ER_ERR_ALIGN;
-  const int mpad = mpad_of(M), uk = uk_of(mpad);
-  if (workspace_bytes < workspace_for(mpad)) return ER_ERR_WORKSPACE;
+  if (workspace_bytes < workspace_for(mpad_of(M))) return ER_ERR_WORKSPACE;
   int st = er::check_arch();
   if (st != ER_OK) return st;
-
-  // plan: stream-K over one CTA per SM; beyond the counter array whole tiles are dealt out (no partial sums)
+  const BPlan pl = bf16_plan(M, N, K);
+  const int mpad = pl.mpad, uk = uk_of(mpad);
   const int mchunks = (int)((M + mpad - 1) / mpad), ntiles = (int)(N / kTileN);
   const long long tiles = (long long)ntiles * mchunks;
   const int G = (int)(K / uk);
   if (tiles * G >= (1ll << 31)) return ER_ERR_SHAPE;
-  const int unit_groups = (tiles <= ER_GEMM_COUNTER_BYTES / 4) ? 1 : G;
+  const int unit_groups = pl.whole ? G : 1;
   const long long units = tiles * G / unit_groups;
-  int ctas = er::sm_count();
-  if (er::g_tune.force_ctas > 0 && er::g_tune.force_ctas < ctas) ctas = er::g_tune.force_ctas;
-  if ((long long)ctas > units) ctas = (int)units;
+  const int ctas = pl.ctas;
 
   CUtensorMap mw, mx;
   const bool ok = er::make_map_2d(&mw, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, w_bf16, (uint64_t)N, (uint64_t)K,
