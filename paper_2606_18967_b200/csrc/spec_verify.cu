@@ -14,11 +14,17 @@
 // reads less when acceptance is low but pays a cluster barrier and a DRAM round trip per position; with the
 // paper's acceptance of ~0.98 every row is needed anyway).  The sweep is bound by the special-function unit
 // (one ex2 per logit, 16 per clock and SM) and by HBM about equally, so everything else in its loop is kept
-// small: the running maximum of a bf16 row is tracked on the packed words (4 max.bf16x2 per 8 logits, no
-// unpacking), and the segments of consecutive rows are dealt to the warps in rotation so that no warp carries
-// the ragged tail of every row.  The residual draw is a multi-level inverse CDF: per-warp segment sums ->
-// per-CTA totals, exchanged -> the CTA whose range holds the threshold does an fp64 blocked prefix over its
-// segments (one warp) and a warp scan inside the one segment that contains the threshold.
+// small: the maximum of a chunk of bf16 logits is taken on the packed words (max.bf16x2) and compared with one
+// setp against a threshold (the softmax reference of a lane is raised lazily, see Acc), and the segments of
+// consecutive rows are dealt to the warps in rotation so that no warp carries the ragged tail of every row.
+// The residual draw is a multi-level inverse CDF: per-warp segment sums -> per-CTA totals, exchanged -> the
+// CTA whose range holds the threshold does an fp64 blocked prefix over its segments (one warp) and a warp scan
+// inside the one segment that contains the threshold.
+//
+// Two kernels share that decomposition: spec_verify_ring_kernel (logits whose rows are 16-byte multiples: every
+// paper-shaped workload) streams the rows through a shared-memory ring filled by one producer lane with
+// cp.async.bulk; spec_verify_kernel reads them with ld.global batches into registers (probability inputs, rows
+// that are not 16-byte multiples).
 #include <cooperative_groups.h>
 #include <cuda_bf16.h>
 #include "er_common.cuh"
@@ -39,13 +45,13 @@ constexpr int kMaxV = 1 << 20;
 constexpr float kNegInf = -3.0e38f;
 
 // ---- 8 consecutive elements starting at token v0 (clipped to V): raw load, then widening to fp32 ----
-// (split in two so that the loads of several tiles can be in flight before the first one is consumed)
+// (split in two so that the loads of several segments can be in flight before the first one is consumed)
 template <typename T>
 struct Load8;
 template <>
 struct Load8<float> {
   struct Raw { float4 a, b; };
-  static constexpr int kBatch = 2;   // tiles whose loads are issued together
+  static constexpr int kBatch = 2;   // segments whose loads are issued together (register path)
   static __device__ __forceinline__ Raw load(const float* row, int v0, int V, bool vec, float fill) {
     Raw r;
     if (vec && v0 + 8 <= V) {
