@@ -17,6 +17,9 @@ Parity pins (tests/test_oracle_*.py, `-m "not gpu"`):
   w4a16_gemm      pinned: one-hot read-out, exact-integer probe, pure-Python
                   Fraction brute force on tiny shapes, K-split invariance.
   bf16_gemm       pinned: pure-Python Fraction brute force, exact-integer case, one-hot read-out.
+  quantize_codes8 / pack_codes8 / w8a16_gemm (W8A16)  pinned: |w - q s| <= s/2 in exact
+                  arithmetic, brute force over bf16 values against Fractions, plane identity 16 a + b = q + 128,
+                  round trip, the sum of two W4-oracle contractions plus the 8 s sum(x) term, Fraction brute force.
   spec_verify     pinned: q = p accepts everything, one-hot / zero-probability
                   cases, exact rational enumeration showing the output
                   distribution equals p (the theorem of ref. [29] the paper
@@ -167,6 +170,75 @@ def w4a16_gemm(x_u16: np.ndarray, qweight: np.ndarray, scales_u16: np.ndarray, g
     (a library primitive used as one step, no blocking or reordering of ours)."""
     x = bf16_to_f32(x_u16).astype(np.float64)
     return x @ dequantize(qweight, scales_u16, group).T
+
+
+
+# ----------------------------------------------------------------------------
+# (f3) W8A16 drafter (PAPER.md:L400-L413, Table 4 "RTN W8"; SURVEY 8(f) f3).  Same conventions as W4 with 127 in
+#      place of 7; readings (DESIGN.md W1-W3): symmetric, group 128, bf16 scale = bf16_RNE(amax / 127), codes
+#      clamped to [-127, 127]; stored as TWO nibble planes per group in the W4 layout, so that the W4 kernels can
+#      contract it: q + 128 = 16 a + b, a, b in [0, 15].
+# ----------------------------------------------------------------------------
+QMAX8 = 127
+
+
+def quantize_codes8(w_u16: np.ndarray, group: int = GROUP):
+    """bf16 W[N][K] -> (codes int16 [N][K] in [-127, 127], scales uint16 bf16 bits [K/group][N]); per group:
+    s = bf16_RNE(fp32(amax) / fp32(127)), q = clamp(rint(fp32(w) / fp32(s)), -127, 127), s == 0 -> q = 0."""
+    w_u16 = np.asarray(w_u16, dtype=np.uint16)
+    N, K = w_u16.shape
+    assert K % group == 0
+    G = K // group
+    w = bf16_to_f32(w_u16).reshape(N, G, group)
+    amax = np.max(np.abs(w), axis=2)
+    s_u16 = f32_to_bf16_rne(amax / np.float32(QMAX8))
+    s = bf16_to_f32(s_u16)
+    safe = np.where(s == 0, np.float32(1), s)
+    with np.errstate(invalid="ignore"):
+        ratio = (w / safe[:, :, None]).astype(np.float32)
+    q = np.clip(np.rint(ratio), -QMAX8, QMAX8)
+    q = np.where((s == 0)[:, :, None], np.float32(0), q)
+    s_u16 = np.where(s == 0, np.uint16(0), s_u16)
+    return q.astype(np.int16).reshape(N, K), np.ascontiguousarray(s_u16.T)
+
+
+def pack_codes8(codes8: np.ndarray, scales_u16: np.ndarray, group: int = GROUP):
+    """W8 codes + scales -> the two-plane W4 storage: (qweight uint32 [N][2K/8], scales' bf16 bits [2K/group][N]).
+    Group g of the W8 matrix becomes groups 2g (plane of the high nibbles a, scale 16 s) and 2g + 1 (plane of the low
+    nibbles b, scale s) of a W4 matrix with 2K columns, packed by pack_codes (stored nibble = plane value)."""
+    codes8 = np.asarray(codes8, dtype=np.int32)
+    N, K = codes8.shape
+    G = K // group
+    u = (codes8 + 128).reshape(N, G, group)
+    assert u.min() >= 1 and u.max() <= 255
+    planes = np.stack([u >> 4, u & 15], axis=2)                      # [N][G][2][group], values 0..15
+    codes4 = (planes.reshape(N, 2 * K) - 8).astype(np.int8)          # pack_codes stores q4 + 8 = the plane value
+    s = bf16_to_f32(np.asarray(scales_u16, dtype=np.uint16))         # [G][N]
+    s16 = f32_to_bf16_rne(s * np.float32(16))                        # exact (a power of two) unless it overflows
+    scales2 = np.stack([s16, np.asarray(scales_u16, dtype=np.uint16)], axis=1).reshape(2 * G, N)
+    return pack_codes(codes4), np.ascontiguousarray(scales2)
+
+
+def unpack_codes8(qweight2: np.ndarray, group: int = GROUP) -> np.ndarray:
+    """Inverse of pack_codes8 on the codes: two-plane storage -> int16 codes [N][K] in [-127, 127]."""
+    planes = unpack_codes(qweight2).astype(np.int32) + 8             # [N][2K], values 0..15
+    N, K2 = planes.shape
+    p = planes.reshape(N, K2 // (2 * group), 2, group)
+    return (16 * p[:, :, 0, :] + p[:, :, 1, :] - 128).reshape(N, K2 // 2).astype(np.int16)
+
+
+def quantize_pack8(w_u16: np.ndarray, group: int = GROUP):
+    """The W8 refresh call: bf16 W[N][K] -> (qweight uint32 [N][2K/8] two-plane, scales' bf16 bits [2K/group][N])."""
+    return pack_codes8(*quantize_codes8(w_u16, group), group)
+
+
+def w8a16_gemm(x_u16: np.ndarray, qweight2: np.ndarray, scales2_u16: np.ndarray, group: int = GROUP) -> np.ndarray:
+    """y_ref[m][n] = sum_k double(x[m][k]) * double(q[n][k]) * double(s[k // group][n]), fp64; q from the two planes,
+    s = the low plane's scale (row 2g + 1 of scales')."""
+    x = bf16_to_f32(x_u16).astype(np.float64)
+    q = unpack_codes8(qweight2, group).astype(np.float64)
+    s = bf16_to_f32(np.asarray(scales2_u16, dtype=np.uint16)[1::2]).astype(np.float64)   # [G][N]
+    return x @ (q * np.repeat(s.T, group, axis=1)).T
 
 
 def bf16_gemm(x_u16: np.ndarray, w_u16: np.ndarray) -> np.ndarray:
