@@ -417,6 +417,9 @@ def model_detail(torch, er, I, dev, mode, peak, gammas=(2, 4, 8), Ms=(256, 128, 
     sc = [{n: torch.empty((K // 128, N), dtype=torch.bfloat16, device=dev) for n, N, K in lin} for _ in range(L)]
     lm_head = I.weight_bf16(V, H, I.seed_of("model", "lm_head"), device=dev)
     n_params = sum(N * K for _, N, K in lin) * L
+    # the W8 drafter of Table 4, two nibble planes per group (include/er.h)
+    qw8 = [{n: torch.empty((N, 2 * K // 8), dtype=torch.int32, device=dev) for n, N, K in lin} for _ in range(L)]
+    sc8 = [{n: torch.empty((2 * K // 128, N), dtype=torch.bfloat16, device=dev) for n, N, K in lin} for _ in range(L)]
 
     def refresh_all():
         for l in range(L):
@@ -428,8 +431,17 @@ def model_detail(torch, er, I, dev, mode, peak, gammas=(2, 4, 8), Ms=(256, 128, 
                "frac_of_measured_peak": round(REFRESH_BYTES_PER_ELEM * n_params / refresh_us / 1e3 / peak, 4),
                "floor_ms_at_measured_peak": round(REFRESH_BYTES_PER_ELEM * n_params / peak / 1e6, 3)}
 
+    def refresh8_all():
+        for l in range(L):
+            for n, N, K in lin:
+                er.quantize_pack8(src[l][n], qw8[l][n], sc8[l][n])
+    refresh8_us = _graph_time_us(torch, refresh8_all, 1, mode)
+    w8_refresh_bytes = (2.0 + 1.0 + 4.0 / 128.0) * n_params
+    refresh["w8"] = {"ms": round(refresh8_us / 1e3, 3), "gbs": round(w8_refresh_bytes / refresh8_us / 1e3, 1),
+                     "frac_of_measured_peak": round(w8_refresh_bytes / refresh8_us / 1e3 / peak, 4)}
+
     Mmax = max(Ms) * (max(gammas) + 1)
-    ws = torch.empty(max(er.gemm_workspace_bytes(max(Ms), 2 * FF, H), er.load().er_bf16_gemm_workspace_bytes(Mmax, V, H),
+    ws = torch.empty(max(er.gemm_workspace_bytes(max(Ms), 2 * FF, H), er.load().er_w8_gemm_workspace_bytes(max(Ms), 2 * FF, H), er.load().er_bf16_gemm_workspace_bytes(Mmax, V, H),
                          er.load().er_bf16_gemm_workspace_bytes(Mmax, 2 * FF, H)), dtype=torch.uint8, device=dev)
     er._check(er.load().er_gemm_workspace_init(ws.data_ptr(), ws.numel(), torch.cuda.current_stream().cuda_stream), "ws")
 
@@ -453,6 +465,7 @@ def model_detail(torch, er, I, dev, mode, peak, gammas=(2, 4, 8), Ms=(256, 128, 
         return layers(h, lambda l, n, x: {"qkv": zq, "o": zo, "gate_up": zg, "down": zd}[n])
 
     w4 = lambda l, n, x: er.w4a16_gemm(x, qw[l][n], sc[l][n], workspace=ws)
+    w8 = lambda l, n, x: er.w8a16_gemm(x, qw8[l][n], sc8[l][n], workspace=ws)
     bf = lambda l, n, x: er.bf16_gemm(x, src[l][n], workspace=ws)
     w4_bytes = W4_BYTES_PER_WEIGHT * n_params
     lm_bytes = 2.0 * V * H
@@ -465,6 +478,7 @@ def model_detail(torch, er, I, dev, mode, peak, gammas=(2, 4, 8), Ms=(256, 128, 
         t_glue = _graph_time_us(torch, lambda: glue_only(h0), 1, mode)
         t_lm = _graph_time_us(torch, lambda: er.bf16_gemm(h0, lm_head, workspace=ws), 1, mode)
         t_p = _graph_time_us(torch, lambda: er.bf16_gemm(layers(h0, bf), lm_head, workspace=ws), 1, mode)
+        t_layers8 = _graph_time_us(torch, lambda: layers(h0, w8), 1, mode)
         row = {"M": M, "drafter_w4_layers_us": round(t_layers, 1), "glue_only_us": round(t_glue, 1),
                "lm_head_bf16_us": round(t_lm, 1),
                "w4_gbs_excl_glue": round(w4_bytes / max(t_layers - t_glue, 1e-3) / 1e3, 1),
@@ -472,7 +486,12 @@ def model_detail(torch, er, I, dev, mode, peak, gammas=(2, 4, 8), Ms=(256, 128, 
                "T_q_us": round(t_layers + t_lm, 1),
                "T_q_gbs": round((w4_bytes + lm_bytes) / (t_layers + t_lm) / 1e3, 1),
                "T_q_floor_us_at_measured_peak": round((w4_bytes + lm_bytes) / peak / 1e3, 1),
-               "T_p_us": round(t_p, 1), "per_gamma": []}
+               "T_p_us": round(t_p, 1),
+               "Tq_over_Tp": round((t_layers + t_lm) / t_p, 3),
+               "w8_drafter_layers_us": round(t_layers8, 1), "w8_T_q_us": round(t_layers8 + t_lm, 1),
+               "w8_Tq_over_Tp": round((t_layers8 + t_lm) / t_p, 3),
+               "table4_idealized": {"w4": 0.360, "w8": 0.573, "source": "PAPER.md:L402-L405 (A100, memory-bound model)"},
+               "per_gamma": []}
         for gamma in gammas:
             tgt, _ = I.verify_logits_bf16_device(M, gamma, V, I.seed_of("model", "tgt", M, gamma), dev)
             drf = torch.empty((M, gamma, V), dtype=torch.bfloat16, device=dev)

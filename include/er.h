@@ -157,6 +157,25 @@ int er_bf16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, co
                  int64_t ldw_elems, void* y, int64_t ldy_elems, int y_dtype, void* workspace, size_t workspace_bytes,
                  void* stream);
 
+/* (1') and (2') W8A16 drafter (Table 4 "RTN W8": the more accurate, twice as heavy
+ * drafter).  RTN int8, symmetric, group 128 along K, s = bf16_rne(fp32(amax) / 127), q = clamp(rint(fp32(w) / fp32(s)),
+ * -127, 127), IEEE division, ties to even; s == 0 -> q = 0 (readings W1-W3).
+ *   Storage: TWO NIBBLE PLANES in the W4 layout.  With q + 128 = 16 a + b (a, b in [0, 15]), group g of the matrix becomes
+ *   groups 2g (stored nibbles a) and 2g + 1 (stored nibbles b) of an ER_PACK_V2 matrix with 2 K columns:
+ *   qweight_out  N * K bytes (N * 2K / 8 words), scales_out  bf16 [2K/128][N] with rows (16 s_g, s_g) -- 1 + 4/128 bytes per
+ *   weight.  er_unpack_codes(qweight, N, 2 K) returns the planes as (a - 8, b - 8).
+ *   er_w8a16_gemm: Y = X . dequant^T with q * s never rounded: the W4 per-group kernel contracts both planes of a group
+ *   against the same 128 columns of X with fp32 accumulation and applies the fp32 scales 16 s and s to the two partial
+ *   sums; the offset of the stored nibbles (128 sum_k x) is removed on the fp32 sums.  Every M >= 1 (M > 64 in chunks of 64
+ *   rows).  Workspace: er_w8_gemm_workspace_bytes, counters zeroed once (er_gemm_workspace_init), shared with er_w4a16_gemm
+ *   if large enough for both.  Arguments, alignment, errors, determinism as for er_quantize_pack / er_w4a16_gemm. */
+int er_quantize_pack8(const void* w_bf16, int64_t N, int64_t K, int64_t ldw_elems, int group, void* qweight_out,
+                      void* scales_out, void* stream);
+size_t er_w8_gemm_workspace_bytes(int64_t M, int64_t N, int64_t K);
+int er_w8a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, const void* qweight, const void* scales,
+                  int64_t N, int group, void* y, int64_t ldy_elems, int y_dtype, void* workspace, size_t workspace_bytes,
+                  void* stream);
+
 /* (3) Speculative-decoding verification, one result per sequence b < B.
  *   target  [B][gamma+1][V]  (row gamma = bonus position), draft [B][gamma][V]; contiguous, 16-byte aligned
  *   in_dtype / inputs_are_logits: (ER_F32, 0) = fp32 probabilities; (ER_BF16, 1) and (ER_F32, 1) = logits,

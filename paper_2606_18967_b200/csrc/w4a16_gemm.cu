@@ -114,11 +114,11 @@ __device__ __forceinline__ uint32_t lop3_and_or(uint32_t a, uint32_t mask, uint3
 // busier one: at N >= 32 the eight constant-tile MMAs per group cost more than the subtracts, which issue on the
 // FMA pipe beside the logic-pipe shifts and lop3s).
 template <bool kSub>
-__device__ __forceinline__ void dequant_word(uint32_t w, uint32_t* a) {
+__device__ __forceinline__ void dequant_word(uint32_t w, uint32_t* a, uint32_t off2) {
 #pragma unroll
   for (int t = 0; t < 4; ++t) {
     const uint32_t v = lop3_and_or(w >> (4 * t), 0x000F000Fu, 0x43004300u);
-    if (kSub) asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(a[t]) : "r"(v), "r"(0x3F803F80u), "r"(0xC308C308u));
+    if (kSub) asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(a[t]) : "r"(v), "r"(0x3F803F80u), "r"(off2));
     else a[t] = v;
   }
 }
@@ -146,7 +146,7 @@ __device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("ba
 
 __device__ __forceinline__ void named_bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
-template <int MPAD, bool kClusterMode>
+template <int MPAD, bool kClusterMode, bool kPlanes = false>
 __global__ void __launch_bounds__(kThreads, 1)
 w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
   using C = Cfg<MPAD>;
@@ -227,8 +227,9 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
         mbar_arrive_expect_tx(&full[s], C::kTxBytes);
         // ER_PACK_V2: the [128 rows x 128 k] block of (tile, g) is 8 KiB of contiguous, pre-swizzled bytes
         bulk_load_1d(st, p.qweight + ((size_t)tn * p.G + g) * kWBytes, kWBytes, &full[s], kEvictFirst);
-        tma_load_2d(st + kWBytes, &map_x, &full[s], g * 128, mc * MPAD, kEvictLast);
-        tma_load_2d(st + kWBytes + MPAD * 128, &map_x, &full[s], g * 128 + 64, mc * MPAD, kEvictLast);
+        const int xk = (g >> (kPlanes ? 1 : 0)) * 128;      // two-plane W8: both planes of a group contract the same X columns
+        tma_load_2d(st + kWBytes, &map_x, &full[s], xk, mc * MPAD, kEvictLast);
+        tma_load_2d(st + kWBytes + MPAD * 128, &map_x, &full[s], xk + 64, mc * MPAD, kEvictLast);
         bulk_load_1d(st + kWBytes + C::kXBytes, p.scales + ((size_t)g * p.N + tn * kTileN) * 2, kScaleBytes,
                      &full[s], kEvictFirst);
       }
@@ -265,10 +266,15 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
               const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
               mma_ts_f16(d_t, a_t + kk * 8, bdesc, idesc, kk > 0 ? 1u : 0u);
             }
+            // - 136 * sum_k x[m][k]: the stored nibble's offset.  Two-plane W8: the high-nibble plane (even groups; G is
+            // even, so the parity of gb + it is the plane) carries none, the low-nibble plane all of it (- 2304, see the
+            // constant tile)
+            if (!C::kSubInWorkers && !(kPlanes && !((gb + it) & 1))) {
 #pragma unroll
-            for (int kk = 0; kk < (C::kSubInWorkers ? 0 : 8); ++kk) {   // - 136 * sum_k x[m][k]: the stored nibble's offset
-              const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
-              mma_ts_f16(d_t, tmem + C::kTmemConst + set * 8, bdesc, idesc, 1u);
+              for (int kk = 0; kk < 8; ++kk) {
+                const uint64_t bdesc = smem_desc_sw128(xbase + (kk >> 2) * (MPAD * 128) + (kk & 3) * 32);
+                mma_ts_f16(d_t, tmem + C::kTmemConst + set * 8, bdesc, idesc, 1u);
+              }
             }
             tc_commit(&done[bi]);
             tc_commit(&empty[s]);
@@ -308,7 +314,9 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
 
     if (half == 0) {                       // the set's constant A tile (-136, -136), one lane quarter per warp; ordered
                                            // before the set's first MMA by its first a_full arrival
-      const uint32_t c = 0xC308C308u;
+      // (-136, -136); two-plane W8: (-2304, -2304) = -(16 * 128 + 128 + 128), exact in bf16: with scales (16 s, s) the
+      // planes then sum to s * sum_k x (16 a + b - 128) = s * sum_k x q
+      const uint32_t c = kPlanes ? 0xC510C510u : 0xC308C308u;
       asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%1,%1,%1,%1,%1,%1,%1};" ::"r"(
                        tmem + lane_addr + C::kTmemConst + set * 8), "r"(c) : "memory");
       asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
@@ -380,15 +388,17 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
           const uint4 pk0 = lds128(st + w_addr0);
           const uint4 pk1 = lds128(st + w_addr1);
           const uint32_t sc16 = lds_u16(st + sc_addr);
+          // (-136, -136) as bf16 pair; two-plane W8: the low-nibble plane (odd groups) takes (-128, -128): b - 0
+          const uint32_t off2 = (kPlanes && ((gb + my) & 1)) ? 0xC300C300u : 0xC308C308u;
           uint32_t a[32];
-          dequant_word<C::kSubInWorkers>(pk0.x, a + 0);
-          dequant_word<C::kSubInWorkers>(pk0.y, a + 4);
-          dequant_word<C::kSubInWorkers>(pk0.z, a + 8);
-          dequant_word<C::kSubInWorkers>(pk0.w, a + 12);
-          dequant_word<C::kSubInWorkers>(pk1.x, a + 16);
-          dequant_word<C::kSubInWorkers>(pk1.y, a + 20);
-          dequant_word<C::kSubInWorkers>(pk1.z, a + 24);
-          dequant_word<C::kSubInWorkers>(pk1.w, a + 28);
+          dequant_word<C::kSubInWorkers>(pk0.x, a + 0, off2);
+          dequant_word<C::kSubInWorkers>(pk0.y, a + 4, off2);
+          dequant_word<C::kSubInWorkers>(pk0.z, a + 8, off2);
+          dequant_word<C::kSubInWorkers>(pk0.w, a + 12, off2);
+          dequant_word<C::kSubInWorkers>(pk1.x, a + 16, off2);
+          dequant_word<C::kSubInWorkers>(pk1.y, a + 20, off2);
+          dequant_word<C::kSubInWorkers>(pk1.z, a + 24, off2);
+          dequant_word<C::kSubInWorkers>(pk1.w, a + 28, off2);
           // the set's previous group: its MMAs had this whole conversion to finish; after this the A buffer
           // (read by those MMAs) and the accumulator are free again
           if (!C::kEpiFirst && npend == kBuf) read_back();
@@ -654,12 +664,12 @@ size_t workspace_for(int mpad) {
 }
 
 
-template <int MPAD, bool kCl>
+template <int MPAD, bool kCl, bool kPlanes = false>
 int launch(const CUtensorMap& mx, const GemmParams& gp, const Plan& pl, cudaStream_t stream) {
   static bool attr_set[er::kMaxDevices] = {};
   const int dev = er::current_device();
   if (dev < 0 || dev >= er::kMaxDevices || !attr_set[dev]) {
-    ER_CUDA_TRY(cudaFuncSetAttribute(w4a16_gemm_kernel<MPAD, kCl>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+    ER_CUDA_TRY(cudaFuncSetAttribute(w4a16_gemm_kernel<MPAD, kCl, kPlanes>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                      Cfg<MPAD>::kSmem));
     if (dev >= 0 && dev < er::kMaxDevices) attr_set[dev] = true;
   }
@@ -680,7 +690,7 @@ int launch(const CUtensorMap& mx, const GemmParams& gp, const Plan& pl, cudaStre
     attr[1].val.clusterDim.z = 1;
     cfg.numAttrs = 2;
   }
-  ER_CUDA_TRY(cudaLaunchKernelEx(&cfg, w4a16_gemm_kernel<MPAD, kCl>, mx, gp));
+  ER_CUDA_TRY(cudaLaunchKernelEx(&cfg, w4a16_gemm_kernel<MPAD, kCl, kPlanes>, mx, gp));
   return ER_OK;
 }
 
@@ -747,9 +757,10 @@ int er_gemm_workspace_init(void* workspace, size_t workspace_bytes, void* stream
   return ER_OK;
 }
 
-int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, const void* qweight,
-                  const void* scales, int64_t N, int group, void* y, int64_t ldy_elems, int y_dtype, void* workspace,
-                  size_t workspace_bytes, void* stream) {
+// `planes` = 1: W8 stored as two nibble planes (er_w8a16_gemm): the packed matrix has 2 K columns (2 K / 128 groups), X has K.
+static int gemm_impl(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, const void* qweight,
+                     const void* scales, int64_t N, int group, void* y, int64_t ldy_elems, int y_dtype, void* workspace,
+                     size_t workspace_bytes, void* stream, int planes) {
   if (!x_bf16 || !qweight || !scales || !y) return ER_ERR_NULL;
   if (group != ER_GROUP || M < 1 || M > (1 << 20) || N < kTileN || N % kTileN != 0 || N > (1 << 24) ||
       K < ER_GROUP || K % ER_GROUP != 0 || K > (1 << 24) || ldx_elems < K || ldy_elems < N)
@@ -759,14 +770,15 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
     return ER_ERR_ALIGN;
   if (!workspace) return ER_ERR_WORKSPACE;
   if (!er::aligned16(workspace)) return ER_ERR_ALIGN;
-  const Plan pl = make_plan(M, N, K);
+  const int64_t Kw = planes ? 2 * K : K;           // columns of the packed matrix
+  const Plan pl = make_plan(M, N, Kw);
   if ((long long)pl.tiles * pl.G >= (1ll << 31)) return ER_ERR_SHAPE;
-  if (workspace_bytes < er_gemm_workspace_bytes(M, N, K)) return ER_ERR_WORKSPACE;
+  if (workspace_bytes < er_gemm_workspace_bytes(M, N, Kw)) return ER_ERR_WORKSPACE;
   int st = er::check_arch();
   if (st != ER_OK) return st;
 
   GemmParams gp;
-  gp.M = (int)M; gp.N = (int)N; gp.K = (int)K;
+  gp.M = (int)M; gp.N = (int)N; gp.K = (int)Kw; gp.planes = planes;
   gp.G = pl.G; gp.ntiles = pl.ntiles; gp.tiles = pl.tiles; gp.unit_groups = pl.unit_groups; gp.units = (int)pl.units;
   gp.uq = (int)(pl.units / pl.ctas); gp.ur = (int)(pl.units % pl.ctas);
   gp.split = pl.split;
@@ -779,11 +791,11 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
   gp.partials = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + ER_GEMM_COUNTER_BYTES);
   cudaStream_t s = (cudaStream_t)stream;
   // M > 16: weights dequantised once per tile for all rows, pre-scaled (w4a16_gemm_large.cu)
-  if (M > 16 && (er::g_tune.large == 2 || (er::g_tune.large == 1 && er::large_preferred(M, N, K))))
+  if (!planes && M > 16 && (er::g_tune.large == 2 || (er::g_tune.large == 1 && er::large_preferred(M, N, K))))
     return er::launch_large(x_bf16, M, N, K, ldx_elems, gp, s);
   // M <= 8 on a plan without a cluster (the large-N linears: gate/up): the warp-level-MMA kernel streams them faster
   // (w4a16_gemm_small.cu; measured in profiles/r02_gemm.md)
-  if (M <= 8 && pl.cluster == 1 && er::g_tune.small_mma) return er::launch_small(x_bf16, M, K, ldx_elems, gp, pl, s);
+  if (!planes && M <= 8 && pl.cluster == 1 && er::g_tune.small_mma) return er::launch_small(x_bf16, M, K, ldx_elems, gp, pl, s);
 
   CUtensorMap mx;
   bool ok = er::make_map_2d(&mx, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, x_bf16, (uint64_t)M, (uint64_t)K,
@@ -792,9 +804,30 @@ int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
     er::set_last_cuda_error((int)cudaErrorInvalidValue);
     return ER_ERR_CUDA;
   }
+  if (planes) {     // the two-plane W8 instantiations (er_w8a16_gemm)
+    if (pl.mpad == 16) return pl.cluster > 1 ? launch<16, true, true>(mx, gp, pl, s) : launch<16, false, true>(mx, gp, pl, s);
+    if (pl.mpad == 32) return pl.cluster > 1 ? launch<32, true, true>(mx, gp, pl, s) : launch<32, false, true>(mx, gp, pl, s);
+    return launch<64, false, true>(mx, gp, pl, s);
+  }
   if (pl.mpad == 16) return pl.cluster > 1 ? launch<16, true>(mx, gp, pl, s) : launch<16, false>(mx, gp, pl, s);
   if (pl.mpad == 32) return pl.cluster > 1 ? launch<32, true>(mx, gp, pl, s) : launch<32, false>(mx, gp, pl, s);
   return launch<64, false>(mx, gp, pl, s);
+}
+
+int er_w4a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, const void* qweight,
+                  const void* scales, int64_t N, int group, void* y, int64_t ldy_elems, int y_dtype, void* workspace,
+                  size_t workspace_bytes, void* stream) {
+  return gemm_impl(x_bf16, M, K, ldx_elems, qweight, scales, N, group, y, ldy_elems, y_dtype, workspace, workspace_bytes,
+                   stream, 0);
+}
+
+size_t er_w8_gemm_workspace_bytes(int64_t M, int64_t N, int64_t K) { return er_gemm_workspace_bytes(M, N, 2 * K); }
+
+int er_w8a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, const void* qweight,
+                  const void* scales, int64_t N, int group, void* y, int64_t ldy_elems, int y_dtype, void* workspace,
+                  size_t workspace_bytes, void* stream) {
+  return gemm_impl(x_bf16, M, K, ldx_elems, qweight, scales, N, group, y, ldy_elems, y_dtype, workspace, workspace_bytes,
+                   stream, 1);
 }
 
 }  // extern "C"

@@ -22,6 +22,8 @@ struct GemmParams {
   int uq, ur;          // units / CTAs and units % CTAs: CTA c owns units [c*uq + min(c, ur), ...)
   int split;           // > 0: tile split (see range_begin); uq = groups per tile
   int cluster;         // > 1: the `split` CTAs of a tile form one thread-block cluster and reduce through DSMEM
+  int planes;          // 1: W8 stored as two nibble planes (er_w8a16_gemm): groups 2g, 2g + 1 share the X of group g,
+                       // the even (high-nibble) plane carries no offset, the odd one the whole of it (w4a16_gemm.cu)
   int y_f32;
   int64_t ldy;
   void* y;

@@ -62,6 +62,12 @@ def _bind(lib: ctypes.CDLL) -> ctypes.CDLL:
     lib.er_quantize_pack_batched.argtypes = [ctypes.POINTER(LinearDesc), ctypes.c_int, ctypes.c_int, vp]
     lib.er_w4a16_gemm.restype = ctypes.c_int
     lib.er_w4a16_gemm.argtypes = [vp, i64, i64, i64, vp, vp, i64, ctypes.c_int, vp, i64, ctypes.c_int, vp, sz, vp]
+    lib.er_quantize_pack8.restype = ctypes.c_int
+    lib.er_quantize_pack8.argtypes = [vp, i64, i64, i64, ctypes.c_int, vp, vp, vp]
+    lib.er_w8_gemm_workspace_bytes.restype = sz
+    lib.er_w8_gemm_workspace_bytes.argtypes = [i64, i64, i64]
+    lib.er_w8a16_gemm.restype = ctypes.c_int
+    lib.er_w8a16_gemm.argtypes = [vp, i64, i64, i64, vp, vp, i64, ctypes.c_int, vp, i64, ctypes.c_int, vp, sz, vp]
     lib.er_w4a16_gemm_simt.restype = ctypes.c_int
     lib.er_w4a16_gemm_simt.argtypes = [vp, i64, i64, i64, vp, vp, i64, ctypes.c_int, vp, i64, ctypes.c_int, vp]
     lib.er_bf16_gemm_workspace_bytes.restype = sz
@@ -217,6 +223,44 @@ def w4a16_gemm(x: torch.Tensor, qweight: torch.Tensor, scales: torch.Tensor, out
     _check(lib.er_w4a16_gemm(x.data_ptr(), M, K, x.stride(0), qweight.data_ptr(), scales.data_ptr(), N, GROUP,
                              y.data_ptr(), y.stride(0), ydt, workspace.data_ptr(), workspace.numel(), _stream(x)),
            "er_w4a16_gemm")
+    return y
+
+
+def quantize_pack8(w: torch.Tensor, qweight: torch.Tensor | None = None, scales: torch.Tensor | None = None):
+    """W8 refresh: bf16 W[N][K] -> (qweight int32 [N][2K/8]: two nibble planes in the W4 layout, scales bf16 [2K/128][N]:
+    rows (16 s_g, s_g)); include/er.h."""
+    _cuda(w, "w")
+    assert w.dtype == torch.bfloat16 and w.dim() == 2 and w.stride(1) == 1
+    N, K = w.shape
+    if qweight is None:
+        qweight = torch.empty((N, 2 * K // 8), dtype=torch.int32, device=w.device)
+    if scales is None:
+        scales = torch.empty((2 * K // GROUP, N), dtype=torch.bfloat16, device=w.device)
+    _check(load().er_quantize_pack8(w.data_ptr(), N, K, w.stride(0), GROUP, qweight.data_ptr(), scales.data_ptr(),
+                                    _stream(w)), "er_quantize_pack8")
+    return qweight, scales
+
+
+def w8a16_gemm(x: torch.Tensor, qweight: torch.Tensor, scales: torch.Tensor, out_dtype=torch.bfloat16,
+               y: torch.Tensor | None = None, workspace: torch.Tensor | None = None):
+    """Y[M][N] = X[M][K] . dequant(two-plane qweight, scales)[N][K]^T (er_w8a16_gemm)."""
+    _cuda(x, "x")
+    assert x.dtype == torch.bfloat16 and x.dim() == 2 and x.stride(1) == 1
+    M, K = x.shape
+    N = qweight.shape[0]
+    if y is None:
+        y = torch.empty((M, N), dtype=out_dtype, device=x.device)
+    ydt = ER_F32 if y.dtype == torch.float32 else ER_BF16
+    lib = load()
+    if workspace is None:
+        nbytes = lib.er_w8_gemm_workspace_bytes(M, N, K)
+        if nbytes == 0:
+            raise ErError(2, "er_w8_gemm_workspace_bytes")
+        workspace = torch.empty(nbytes, dtype=torch.uint8, device=x.device)
+        _check(lib.er_gemm_workspace_init(workspace.data_ptr(), nbytes, _stream(x)), "er_gemm_workspace_init")
+    _check(lib.er_w8a16_gemm(x.data_ptr(), M, K, x.stride(0), qweight.data_ptr(), scales.data_ptr(), N, GROUP,
+                             y.data_ptr(), y.stride(0), ydt, workspace.data_ptr(), workspace.numel(), _stream(x)),
+           "er_w8a16_gemm")
     return y
 
 
