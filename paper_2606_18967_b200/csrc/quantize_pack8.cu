@@ -22,10 +22,40 @@ __device__ __forceinline__ uint32_t absmax2(uint32_t a, uint32_t b) {
   return d;
 }
 
-// stored byte u = q + 128 of one weight (s > 0)
-__device__ __forceinline__ uint32_t code8(float w, float s) {
-  const float t = fminf(fmaxf(rintf(__fdiv_rn(w, s)), -127.0f), 127.0f);
-  return (uint32_t)((int)t + 128);
+constexpr float kMagic8 = 12582912.0f + 128.0f;   // 1.5 * 2^23 + 128: bits(t + kMagic8) = 0x4B400000 + rint(t) + 128
+
+// bits whose low byte is the stored code u = clamp(rint(w / s), -127, 127) + 128.  r ~ 1 / s (MUFU.RCP) and one
+// exact-residual Newton step, as in quantize_pack.cu: the result is the IEEE quotient wherever that matters -- exact at
+// ties (k + 1/2 is representable), and a non-tie quotient of two 8-bit significands with |w / s| >= 1/2 is at least
+// 1/1020 away from a tie, against an error of t below 2e-5.  kDiv: plain IEEE division (denormal scales, 1 / s overflows).
+template <bool kDiv>
+__device__ __forceinline__ uint32_t code8(float w, float s, float r) {
+  float t;
+  if (kDiv) {
+    t = __fdiv_rn(w, s);
+  } else {
+    t = w * r;
+    const float e = __fmaf_rn(-t, s, w);
+    t = __fmaf_rn(e, r, t);
+  }
+  return __float_as_uint(fminf(fmaxf(t, -127.0f), 127.0f) + kMagic8);
+}
+
+// The two plane words of 8 consecutive k (4 raw words of bf16 pairs): logical k = 2 t + h sits in nibble t + 4 h.
+template <bool kDiv>
+__device__ __forceinline__ void planes8(const uint32_t* raw, float s, float r, uint32_t& hi, uint32_t& lo) {
+  uint32_t a = 0, b = 0;
+#pragma unroll
+  for (int t = 0; t < 4; ++t) {
+    const uint32_t u0 = code8<kDiv>(__uint_as_float(raw[t] << 16), s, r);
+    const uint32_t u1 = code8<kDiv>(__uint_as_float(raw[t] & 0xFFFF0000u), s, r);
+    a |= ((u0 >> 4) & 15u) << (4 * t);
+    a |= ((u1 >> 4) & 15u) << (4 * t + 16);
+    b |= (u0 & 15u) << (4 * t);
+    b |= (u1 & 15u) << (4 * t + 16);
+  }
+  hi = a;
+  lo = b;
 }
 
 __global__ void __launch_bounds__(kThreads) quantize_pack8_kernel(const uint16_t* __restrict__ w, int64_t N, int64_t K,
@@ -65,22 +95,14 @@ __global__ void __launch_bounds__(kThreads) quantize_pack8_kernel(const uint16_t
     const float s = __bfloat162float(sb);
     // plane words: the 8 codes of a word sit at nibble t + 4 h for logical k = 2 t + h (as in the W4 layout)
     uint32_t hi[2] = {0x88888888u, 0x88888888u}, lo[2] = {0u, 0u};    // s == 0: q = 0 -> u = 128 = (8, 0)
-    if (s > 0.0f) {
-#pragma unroll
-      for (int wd = 0; wd < 2; ++wd) {
-        uint32_t a = 0, b = 0;
-#pragma unroll
-        for (int t = 0; t < 4; ++t) {
-          const uint32_t u0 = code8(__uint_as_float(raw[4 * wd + t] << 16), s);
-          const uint32_t u1 = code8(__uint_as_float(raw[4 * wd + t] & 0xFFFF0000u), s);
-          a |= (u0 >> 4) << (4 * t);
-          a |= (u1 >> 4) << (4 * t + 16);
-          b |= (u0 & 15u) << (4 * t);
-          b |= (u1 & 15u) << (4 * t + 16);
-        }
-        hi[wd] = a;
-        lo[wd] = b;
-      }
+    if (s >= 1e-30f) {
+      float r;
+      asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(s));
+      planes8<false>(raw, s, r, hi[0], lo[0]);
+      planes8<false>(raw + 4, s, r, hi[1], lo[1]);
+    } else if (s > 0.0f) {
+      planes8<true>(raw, s, 0.f, hi[0], lo[0]);
+      planes8<true>(raw + 4, s, 0.f, hi[1], lo[1]);
     }
     if (ok[it]) {
       const int64_t n = n0 + r_in_tile;
