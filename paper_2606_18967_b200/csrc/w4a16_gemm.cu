@@ -3,7 +3,10 @@
 // small batch; L175: W4A16 weight-only kernel; L467: "on-the-fly dequantization and kernel-level overhead").
 // This file: the host entry point (validation, work plan, dispatch to the three kernels) and the tcgen05 kernel with
 // one fp32 accumulator per 128-k group (exact group scale), which serves M <= 16 -- except M <= 8 on plans without a
-// cluster (w4a16_gemm_small.cu) -- and 16 < M <= 64, and larger M where w4a16_gemm_large.cu is not preferred.
+// cluster (w4a16_gemm_small.cu) -- and 16 < M <= 64 (M > 64: w4a16_gemm_large.cu).  Instantiated a second time
+// (kPlanes) for er_w8a16_gemm: a W8 matrix stored as two nibble planes per group (quantize_pack8.cu) is a W4 matrix with
+// 2 K columns whose groups 2g, 2g + 1 contract the same 128 columns of X; the high plane carries no offset, the low plane
+// all of it (M <= 16: constant tile -2304; above: -136 / -128 in the workers).
 //
 // What the earlier versions taught (profiles/r01_*, r02_gemm.md): TMA / MMA issue must be warp-uniform code with one
 // elected lane; a closed ring of few TMEM buffers between separate converter / MMA / read-back roles is bound by the
