@@ -157,6 +157,20 @@ int er_bf16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, co
                  int64_t ldw_elems, void* y, int64_t ldy_elems, int y_dtype, void* workspace, size_t workspace_bytes,
                  void* stream);
 
+/* (1'') er_w4a16_gemm for callers that may not allocate device memory (code under CUDA-graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): same operation, arithmetic and results as er_w4a16_gemm, M <= ER_STATIC_GEMM_MAX_M
+ * (the memory-bound regime), but NO workspace argument -- the tile counters and split-K partial tiles live in a static
+ * device array inside the library (3.2 MB; every GPU that loads the library holds it until exit).  The call allocates
+ * nothing (no cudaMalloc / cudaFree, no allocating library routine) and enqueues one 16 KiB memset of the counters plus
+ * the kernel on `stream`.  All calls on a device share that one array: calls that may OVERLAP on the GPU (different
+ * streams, or graph branches without a dependency) race on it -- keep them ordered.  Errors as er_w4a16_gemm (on an
+ * argument error at most the memset of the library's own counters has been enqueued), plus
+ * ER_ERR_SHAPE for M > ER_STATIC_GEMM_MAX_M and ER_ERR_WORKSPACE on a device whose SM count the array is too small for
+ * (> 192 SMs). */
+#define ER_STATIC_GEMM_MAX_M 16
+int er_w4a16_gemm_static(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, const void* qweight,
+                         const void* scales, int64_t N, int group, void* y, int64_t ldy_elems, int y_dtype, void* stream);
+
 /* (1') and (2') W8A16 drafter (Table 4 "RTN W8": the more accurate, twice as heavy
  * drafter).  RTN int8, symmetric, group 128 along K, s = bf16_rne(fp32(amax) / 127), q = clamp(rint(fp32(w) / fp32(s)),
  * -127, 127), IEEE division, ties to even; s == 0 -> q = 0 (readings W1-W3).

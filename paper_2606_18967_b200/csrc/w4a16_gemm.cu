@@ -833,4 +833,35 @@ int er_w8a16_gemm(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, c
                    stream, 1);
 }
 
+// ---- er_w4a16_gemm_static: the M <= 16 drafter linear for callers that may not allocate (include/er.h) ----
+// The tile counters and split-K partial tiles live in THIS array instead of a caller-provided workspace: 16 KiB of
+// counters + 2 x 16 x 128 fp32 per CTA for up to 192 CTAs.  Every GPU that loads the library holds it until exit.  In
+// host code `g_static_scratch` is only a stand-in for the symbol: its device address is asked for once per device, with
+// that device current, and that pointer is what the kernel gets.
+constexpr size_t kStaticScratchBytes = ER_GEMM_COUNTER_BYTES + (size_t)192 * 2 * ER_STATIC_GEMM_MAX_M * kTileN * sizeof(float);
+static __device__ __align__(256) unsigned char g_static_scratch[kStaticScratchBytes];
+
+int er_w4a16_gemm_static(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems, const void* qweight,
+                         const void* scales, int64_t N, int group, void* y, int64_t ldy_elems, int y_dtype,
+                         void* stream) {
+  if (M > ER_STATIC_GEMM_MAX_M) return ER_ERR_SHAPE;                 // beyond what the static scratch is sized for
+  if (M >= 1 && N >= kTileN && N % kTileN == 0 && K >= ER_GROUP && K % ER_GROUP == 0 &&
+      er_gemm_workspace_bytes(M, N, K) > kStaticScratchBytes)
+    return ER_ERR_WORKSPACE;                                         // a device with more than 192 SMs
+  static void* ptr[er::kMaxDevices];                                 // device address of the array, per device
+  const int dev = er::current_device();
+  if (dev < 0 || dev >= er::kMaxDevices) return ER_ERR_CUDA;
+  if (!ptr[dev]) {
+    void* q = nullptr;
+    ER_CUDA_TRY(cudaGetSymbolAddress(&q, g_static_scratch));
+    if (!q) return ER_ERR_CUDA;
+    ptr[dev] = q;
+  }
+  // The array keeps the last call's contents.  The partial tiles are always written before they are read; the counters
+  // must start at zero: a completed call leaves them so, this memset covers a call that did not complete.
+  ER_CUDA_TRY(cudaMemsetAsync(ptr[dev], 0, ER_GEMM_COUNTER_BYTES, (cudaStream_t)stream));
+  return gemm_impl(x_bf16, M, K, ldx_elems, qweight, scales, N, group, y, ldy_elems, y_dtype, ptr[dev],
+                   kStaticScratchBytes, stream, 0);
+}
+
 }  // extern "C"

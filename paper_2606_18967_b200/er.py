@@ -68,6 +68,8 @@ def _bind(lib: ctypes.CDLL) -> ctypes.CDLL:
     lib.er_w8_gemm_workspace_bytes.argtypes = [i64, i64, i64]
     lib.er_w8a16_gemm.restype = ctypes.c_int
     lib.er_w8a16_gemm.argtypes = [vp, i64, i64, i64, vp, vp, i64, ctypes.c_int, vp, i64, ctypes.c_int, vp, sz, vp]
+    lib.er_w4a16_gemm_static.restype = ctypes.c_int
+    lib.er_w4a16_gemm_static.argtypes = [vp, i64, i64, i64, vp, vp, i64, ctypes.c_int, vp, i64, ctypes.c_int, vp]
     lib.er_w4a16_gemm_simt.restype = ctypes.c_int
     lib.er_w4a16_gemm_simt.argtypes = [vp, i64, i64, i64, vp, vp, i64, ctypes.c_int, vp, i64, ctypes.c_int, vp]
     lib.er_bf16_gemm_workspace_bytes.restype = sz
@@ -223,6 +225,17 @@ def w4a16_gemm(x: torch.Tensor, qweight: torch.Tensor, scales: torch.Tensor, out
     _check(lib.er_w4a16_gemm(x.data_ptr(), M, K, x.stride(0), qweight.data_ptr(), scales.data_ptr(), N, GROUP,
                              y.data_ptr(), y.stride(0), ydt, workspace.data_ptr(), workspace.numel(), _stream(x)),
            "er_w4a16_gemm")
+    return y
+
+
+def w4a16_gemm_static(x: torch.Tensor, qweight: torch.Tensor, scales: torch.Tensor, y: torch.Tensor):
+    """er_w4a16_gemm_static: Y = X . dequant^T at M <= 16 with the scratch in the library's static device array; the
+    caller passes inputs and the output, nothing is allocated here or in the library."""
+    M, K = x.shape
+    N = qweight.shape[0]
+    ydt = ER_F32 if y.dtype == torch.float32 else ER_BF16
+    _check(load().er_w4a16_gemm_static(x.data_ptr(), M, K, x.stride(0), qweight.data_ptr(), scales.data_ptr(), N, GROUP,
+                                       y.data_ptr(), y.stride(0), ydt, _stream(x)), "er_w4a16_gemm_static")
     return y
 
 
