@@ -3,7 +3,7 @@
 // small batch; L175: W4A16 weight-only kernel; L467: "on-the-fly dequantization and kernel-level overhead").
 // This file: the host entry point (validation, work plan, dispatch to the three kernels) and the tcgen05 kernel with
 // one fp32 accumulator per 128-k group (exact group scale), which serves M <= 16 -- except M <= 8 on plans without a
-// cluster (w4a16_gemm_small.cu) -- and 16 < M <= 64 (M > 64: w4a16_gemm_large.cu).  Instantiated a second time
+// cluster (w4a16_gemm_small.cu) -- and every M > 16 (M > 64 in chunks of 64 batch rows).  Instantiated a second time
 // (kPlanes) for er_w8a16_gemm: a W8 matrix stored as two nibble planes per group (quantize_pack8.cu) is a W4 matrix with
 // 2 K columns whose groups 2g, 2g + 1 contract the same 128 columns of X; the high plane carries no offset, the low plane
 // all of it (M <= 16: constant tile -2304; above: -136 / -128 in the workers).
@@ -211,8 +211,11 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   // The producer first asks L2 for the beginning of this CTA's weight stream (a contiguous byte range of ER_PACK_V2):
   // safe even right behind a refresh, because L2 is the point of coherence and a prefetched line cannot be stale.
   if (warp == kProdWarp && elect_one()) {
-    const int npf = n_it < 8 ? n_it : 8;          // 64 KB per SM: deeper prefetches measured slower (profiles/r02_gemm.md)
-    if (npf > 0) bulk_prefetch_l2(p.qweight + (size_t)gb * kWBytes, (uint32_t)npf * kWBytes);
+    // 64 KB per SM: deeper prefetches measured slower (profiles/r02_gemm.md).  With several batch chunks (M > 64) the
+    // tiles of chunk mc reuse the weight blocks of chunk 0: the stream position is gb modulo the blocks of the matrix
+    const int wblocks = p.ntiles * p.G, wb = gb % wblocks;
+    const int npf = min(min(n_it, 8), wblocks - wb);
+    if (npf > 0) bulk_prefetch_l2(p.qweight + (size_t)wb * kWBytes, (uint32_t)npf * kWBytes);
   }
   asm volatile("griddepcontrol.wait;" ::: "memory");
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
@@ -581,7 +584,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
 namespace er {
 
 #ifdef ER_DEV
-Tuning g_tune = {1, 1, 1, 0, 1, 1};
+Tuning g_tune = {1, 1, 1, 0, 1, 0};
 #endif
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -632,9 +635,16 @@ Plan make_plan(int64_t M, int64_t N, int64_t K) {
   pl.G = (int)(K / ER_GROUP);
   // one ticket counter per tile: beyond the counter array, whole tiles are dealt out (no partial sums)
   pl.unit_groups = (pl.tiles <= ER_GEMM_COUNTER_BYTES / 4) ? 1 : pl.G;
-  pl.units = (long long)pl.tiles * pl.G / pl.unit_groups;
   int ctas = er::sm_count();
   if (tn.force_ctas > 0 && tn.force_ctas < ctas) ctas = tn.force_ctas;
+  // M > 64 (several chunks of 64 batch rows, every (chunk, weight tile) a tile of its own): whole tiles when they keep
+  // the CTAs about as busy as stream-K ranges would -- a partial tile is 32 KB there
+  if (pl.mchunks > 1 && tn.force_ctas == 0) {
+    const long long whole = (long long)((pl.tiles + ctas - 1) / ctas) * pl.G;
+    const long long sk = ((long long)pl.tiles * pl.G + ctas - 1) / ctas;
+    if (whole * 100 <= sk * 115) pl.unit_groups = pl.G;
+  }
+  pl.units = (long long)pl.tiles * pl.G / pl.unit_groups;
   if ((long long)ctas > pl.units) ctas = (int)pl.units;
   pl.ctas = ctas;
   // tile split: when k >= 2 parts per tile fill at least 90 % of the CTAs, no CTA has to straddle two tiles
@@ -747,10 +757,13 @@ int er_dev_gemm_tuning(int key, int value) {
 
 size_t er_gemm_workspace_bytes(int64_t M, int64_t N, int64_t K) {
   if (M < 1 || N < kTileN || N % kTileN != 0 || K < ER_GROUP || K % ER_GROUP != 0) return 0;
-  // the largest over the kernels that may serve this M (the development library can switch between them)
   const size_t exact = workspace_for(mpad_of(M));
+#ifdef ER_DEV   // the development library can switch to the pre-scaled large-batch kernel (w4a16_gemm_large.cu)
   const size_t large = M > 16 ? er::large_workspace_bytes(M, N, K) : 0;
   return exact > large ? exact : large;
+#else
+  return exact;
+#endif
 }
 
 int er_gemm_workspace_init(void* workspace, size_t workspace_bytes, void* stream) {
@@ -793,9 +806,11 @@ static int gemm_impl(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems
   gp.counters = reinterpret_cast<int*>(workspace);
   gp.partials = reinterpret_cast<float*>(reinterpret_cast<uint8_t*>(workspace) + ER_GEMM_COUNTER_BYTES);
   cudaStream_t s = (cudaStream_t)stream;
-  // M > 16: weights dequantised once per tile for all rows, pre-scaled (w4a16_gemm_large.cu)
+#ifdef ER_DEV
+  // development library only: the pre-scaled large-batch kernel (w4a16_gemm_large.cu says why it is not shipped)
   if (!planes && M > 16 && (er::g_tune.large == 2 || (er::g_tune.large == 1 && er::large_preferred(M, N, K))))
     return er::launch_large(x_bf16, M, N, K, ldx_elems, gp, s);
+#endif
   // M <= 8 on a plan without a cluster (the large-N linears: gate/up): the warp-level-MMA kernel streams them faster
   // (w4a16_gemm_small.cu; measured in profiles/r02_gemm.md)
   if (!planes && M <= 8 && pl.cluster == 1 && er::g_tune.small_mma) return er::launch_small(x_bf16, M, K, ldx_elems, gp, pl, s);

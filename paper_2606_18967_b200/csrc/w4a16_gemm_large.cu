@@ -1,13 +1,16 @@
-// w4a16_gemm_large.cu -- er_w4a16_gemm at M > 16: the batches at the head of a rollout, where the drafter linear turns
-// from memory-bound to tensor-bound (ridge at M ~ 54-66 on this box; the compute term only matters
-// at large B).  The M <= 16 kernels (w4a16_gemm.cu, w4a16_gemm_small.cu) keep a fresh fp32 accumulator per 128-k group
-// so that the group scale is applied exactly; that costs a TENSOR-MEMORY read-back of the whole [128 x M] accumulator
-// per group and, at M > 64, a second / third / fourth pass over the weights.  Here the weights are dequantised ONCE per
-// tile for all batch rows and PRE-SCALED: the A operand is bf16_rne(q * s) (q exact in bf16, one rounding by the
-// multiply), one fp32 accumulator in TENSOR MEMORY runs over the whole K range of a tile segment, and nothing is read
-// back until the segment ends.  The rounding of q * s to bf16 costs accuracy the stated tolerance allows
-// (max|d| <= 1e-2 rms + 1e-3 on the fp32 output; measured 0.5-0.6 of it, G1), which is why the exact kernels
-// stay in charge of M <= 16.
+// w4a16_gemm_large.cu -- DEVELOPMENT LIBRARY ONLY (-DER_DEV; not part of liber_b200.so): a pre-scaled large-batch variant of
+// er_w4a16_gemm for M > 16.  The shipped kernels (w4a16_gemm.cu, w4a16_gemm_small.cu) keep a fresh fp32 accumulator per
+// 128-k group so that the group scale is applied exactly; that costs a TENSOR-MEMORY read-back of the whole [128 x M]
+// accumulator per group and, at M > 64, one pass over the weights per 64 batch rows.  Here the weights are dequantised
+// ONCE per tile for all batch rows and PRE-SCALED: the A operand is bf16_rne(q * s) (q exact in bf16, one rounding by the
+// multiply), one fp32 accumulator in TENSOR MEMORY runs over the whole K range of a tile segment, and nothing is read back
+// until the segment ends.  It is 10-25 % faster than the exact kernel at M = 128 / 256 (gate/up 37.8 / 66.2 us against
+// 46.5 / 88.9; profiles/r02_gemm.md section 6) -- and NOT SHIPPED, because the rounding of q * s eats the whole stated
+// tolerance (max|d| <= 1e-2 rms + 1e-3 on the fp32 output): the error of an output is a sum of K independent roundings,
+// sigma ~ 1.6e-3 of that output's own magnitude, so over ~10^6 outputs whose magnitudes differ (outlier channels) the
+// maximum reaches the bound -- measured 1.04 x the bound on config 2's O projection at M = 256 over all columns
+// (tests/test_gpu_config2.py), 0.7-0.9 x on uniformly random nibbles.  Kept for the tests that compare it with the exact
+// path (dev key 7) and as the starting point of an exact two-term variant (q * s = q * s_hi + q * s_lo, both exact in bf16).
 //
 //   persistent   one CTA per SM, stream-K over (tile, 128-k group) units (w4a16_plan.cuh); swap-AB: the 128 weight rows
 //                of a tile are the M of tcgen05.mma.kind::f16, the padded batch (32 ... 256) is its N.
@@ -22,6 +25,7 @@
 //                double-buffered up to M = 128, so the epilogue of a segment runs under the MMAs of the next.
 //   warps 0-3    epilogue: tcgen05.ld (a thread owns a weight row), direct store of whole tiles, fp32 partials to the
 //                workspace otherwise (ticket per tile, ascending CTA order).  Deterministic.
+#ifdef ER_DEV
 #include "w4a16_plan.cuh"
 
 namespace {
@@ -520,3 +524,4 @@ int launch_large(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, Ge
 }
 
 }  // namespace er
+#endif  // ER_DEV

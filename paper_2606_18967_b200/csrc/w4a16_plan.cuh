@@ -76,7 +76,7 @@ struct Tuning {
 #ifdef ER_DEV
 extern Tuning g_tune;
 #else
-constexpr Tuning g_tune = {1, 1, 1, 0, 1, 1};
+constexpr Tuning g_tune = {1, 1, 1, 0, 1, 0};
 #endif
 
 // 2-D row-major tensor [rows][cols] of elements, row pitch in bytes, box [box_rows][box_cols].

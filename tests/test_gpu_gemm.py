@@ -54,16 +54,13 @@ def test_config0(simt):
 
 @pytest.mark.parametrize("simt,rows", [(True, 256), (False, 64), (False, 256)])
 def test_one_hot_reads_out_dequantised_matrix(simt, rows):
-    # x[m] = e_k: y[m][n] must equal the dequantised weight of the kernel that serves this batch size, exactly (pins
-    # layout, dequant, transpose): q[n][k] * s[k//128][n] for M <= 64 (and the SIMT kernel at any M), and that
-    # product rounded to bf16 (RNE) for M > 64, where er.h states that the weights are pre-scaled in bf16
+    # x[m] = e_k: y[m][n] must equal q[n][k] * s[k//128][n] exactly, at every batch size and in both kernels (pins
+    # layout, dequant, transpose, and that q * s is never rounded: the product has up to 12 significant bits)
     N, K = 256, 512
     codes = I.random_codes(N, K, 3)          # includes -8
     su = _random_scales(K // 128, N, 4)
     qw, sc = _dev_weights(codes, su)
-    wd = O.dequantize(O.pack_codes(codes), su)      # [N][K] fp64, exact (<= 12 significant bits)
-    if rows > 64 and not simt:
-        wd = torch.from_numpy(wd).to(torch.float32).to(torch.bfloat16).to(torch.float64).numpy()
+    wd = O.dequantize(O.pack_codes(codes), su)      # [N][K] fp64, exact
     for k0 in range(0, K, rows):
         x = torch.zeros((rows, K), dtype=torch.bfloat16, device=DEV)
         x[torch.arange(rows), k0 + torch.arange(rows)] = 1.0
@@ -170,9 +167,7 @@ def _sampled_columns_check(x, qw, sc, N, K, seed, label, y=None):
     assert err_s <= _tol(y_ref), f"{label} M={M}: SIMT max|d|={err_s}"
     rms = float(y_simt.float().pow(2).mean().sqrt())
     gap = float((y - y_simt).abs().max())
-    # (M > 64 may be served by the large-batch kernel, whose A operand is bf16_rne(q * s): there the gap to the exact
-    # CUDA-core result is the rounding the stated tolerance allows, not a summation-order effect)
-    gap_tol = 1e-4 * rms + 1e-5 if M <= 64 else 1e-2 * rms + 1e-3
+    gap_tol = 1e-4 * rms + 1e-5
     assert gap <= gap_tol, f"{label} M={M}: tensor-core kernel vs SIMT over all columns: {gap} (rms {rms})"
     assert torch.isfinite(y).all()
     return y
