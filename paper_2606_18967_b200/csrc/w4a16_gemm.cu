@@ -211,10 +211,11 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
   // The producer first asks L2 for the beginning of this CTA's weight stream (a contiguous byte range of ER_PACK_V2):
   // safe even right behind a refresh, because L2 is the point of coherence and a prefetched line cannot be stale.
   if (warp == kProdWarp && elect_one()) {
-    // 64 KB per SM: deeper prefetches measured slower (profiles/r02_gemm.md).  With several batch chunks (M > 64) the
-    // tiles of chunk mc reuse the weight blocks of chunk 0: the stream position is gb modulo the blocks of the matrix
-    const int wblocks = p.ntiles * p.G, wb = gb % wblocks;
-    const int npf = min(min(n_it, 8), wblocks - wb);
+    // 64 KB per SM: deeper prefetches measured slower (profiles/r02_gemm.md).  Only with one batch chunk (M <= 64): with
+    // several, the tiles of chunk mc > 0 re-use the weight blocks of chunk 0 and gb is no position in the weight stream
+    // (a prefetch of gb * 8 KiB reached beyond the matrix and cost the M > 64 launches a factor of two)
+    const int npf = p.mchunks == 1 ? (n_it < 8 ? n_it : 8) : 0;
+    const int wb = gb;
     if (npf > 0) bulk_prefetch_l2(p.qweight + (size_t)wb * kWBytes, (uint32_t)npf * kWBytes);
   }
   asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -795,7 +796,7 @@ static int gemm_impl(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems
 
   GemmParams gp;
   gp.M = (int)M; gp.N = (int)N; gp.K = (int)Kw; gp.planes = planes;
-  gp.G = pl.G; gp.ntiles = pl.ntiles; gp.tiles = pl.tiles; gp.unit_groups = pl.unit_groups; gp.units = (int)pl.units;
+  gp.G = pl.G; gp.ntiles = pl.ntiles; gp.mchunks = pl.mchunks; gp.tiles = pl.tiles; gp.unit_groups = pl.unit_groups; gp.units = (int)pl.units;
   gp.uq = (int)(pl.units / pl.ctas); gp.ur = (int)(pl.units % pl.ctas);
   gp.split = pl.split;
   gp.cluster = pl.cluster;

@@ -17,6 +17,7 @@ struct GemmParams {
   int G;               // groups per tile = K / 128
   int ntiles;          // N / 128
   int tiles;           // ntiles * mchunks
+  int mchunks;         // chunks of MPAD batch rows (tile t = chunk t / ntiles of weight tile t % ntiles)
   int unit_groups;     // groups per scheduling unit: 1 (stream-K) or G (whole tiles)
   int units;           // tiles * G / unit_groups (< 2^31, checked on the host)
   int uq, ur;          // units / CTAs and units % CTAs: CTA c owns units [c*uq + min(c, ur), ...)
