@@ -403,3 +403,30 @@ def test_partition_modes_at_m_17_to_32(mode, M):
         y2 = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
         torch.cuda.synchronize()
         assert torch.equal(y1, y2)
+
+@pytest.mark.parametrize("M", [65, 130, 200, 256, 300])
+def test_exact_kernel_above_64_rows_every_plan(M):
+    # M > 64 runs in chunks of 64 batch rows, (chunk, weight tile) = a tile of its own: whole tiles (the automatic plan
+    # here), stream-K ranges whose partial tiles go through the workspace (forced CTA counts), the last chunk ragged;
+    # integer probe: bit-exact against the oracle, i.e. no rounding of q * s at any M
+    N, K = 1024, 1152
+    codes = I.random_codes(N, K, 31)
+    su = np.full((K // 128, N), 0x3F80, dtype=np.uint16)
+    su[1::2] = 0x4000
+    qw, sc = _dev_weights(codes, su)
+    rng = np.random.default_rng(M)
+    x = torch.from_numpy(rng.integers(-1, 3, size=(M, K)).astype(np.float32)).to(DEV).to(torch.bfloat16)
+    ref = O.w4a16_gemm(I.as_u16(x), qw.cpu().numpy().view(np.uint32), su)
+    su2 = _random_scales(K // 128, N, 32)
+    qw2, sc2 = _dev_weights(codes, su2)
+    xg = I.activation_bf16(M, K, I.seed_of("exact64", M), device=DEV)
+    ref2 = O.w4a16_gemm(I.as_u16(xg), qw2.cpu().numpy().view(np.uint32), su2)
+    with er.dev_library() as lib:
+        for ctas in (0, 5, 37, 148):
+            assert lib.er_dev_gemm_tuning(1, ctas) == 0
+            y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
+            y2 = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
+            assert np.array_equal(y.cpu().numpy().astype(np.float64), ref), (M, ctas)
+            assert torch.equal(y, y2)
+            yg = er.w4a16_gemm(xg, qw2, sc2, out_dtype=torch.float32).cpu().numpy().astype(np.float64)
+            assert np.abs(yg - ref2).max() <= 1e-5 * np.sqrt(np.mean(ref2 ** 2)) + 1e-6, (M, ctas)   # fp32 summation only
