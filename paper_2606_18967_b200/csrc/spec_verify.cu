@@ -42,7 +42,10 @@ constexpr int kWarps = kThreads / 32;
 constexpr int kPerThread = 8;
 constexpr int kSeg = 32 * kPerThread;         // 256 tokens: what one warp loads at once
 constexpr int kMaxV = 1 << 20;
-constexpr float kNegInf = -3.0e38f;
+constexpr float kNegInf = -3.0e38f;         // "no finite logit seen yet": the initial reference of the statistics
+// Logit positions beyond V are filled with a true -inf (probability 0), never with a finite sentinel: a finite fill would
+// become the reference of a lane whose real logits are all masked (-inf) and overflow -m * scale
+#define ER_LOGIT_FILL (__uint_as_float(0xFF800000u))
 
 // ---- 8 consecutive elements starting at token v0 (clipped to V): raw load, then widening to fp32 ----
 // (split in two so that the loads of several segments can be in flight before the first one is consumed)
@@ -82,7 +85,7 @@ struct Load8<__nv_bfloat16> {
       r.a = *reinterpret_cast<const uint4*>(row + v0);
     } else {
       uint32_t h[8];
-      const uint32_t fb = __float_as_uint(fill) >> 16;   // the fills used (0, -3e38) survive truncation to bf16
+      const uint32_t fb = __float_as_uint(fill) >> 16;   // the fills used (0, -inf) are exact in bf16
 #pragma unroll
       for (int i = 0; i < 8; ++i)
         h[i] = (v0 + i < V) ? (uint32_t)__bfloat16_as_ushort(row[v0 + i]) : fb;
@@ -304,8 +307,8 @@ __device__ void row_stats(const T* trow, const T* drow, int V, bool vec, float s
       rt[j] = Accum<T>::neg_inf();
       rd[j] = rt[j];
       if (s0 + j * kWarps < nloc && v0 < V) {
-        rt[j] = Load8<T>::load(trow, v0, V, vec, kNegInf);
-        if (drow) rd[j] = Load8<T>::load(drow, v0, V, vec, kNegInf);
+        rt[j] = Load8<T>::load(trow, v0, V, vec, ER_LOGIT_FILL);
+        if (drow) rd[j] = Load8<T>::load(drow, v0, V, vec, ER_LOGIT_FILL);
       }
     }
     Accum<T>::add(rt, at, scale);
@@ -384,7 +387,7 @@ __device__ __forceinline__ void weights8_raw(const typename Load8<T>::Raw& rp, c
 template <typename T, bool kLogits>
 __device__ __forceinline__ void weights8(const T* trow, const T* drow, int v0, int V, bool vec, float scale,
                                          const RowStats& st, const RowStats& sd, bool use_q, float (&w)[8]) {
-  const float fill = kLogits ? kNegInf : 0.f;
+  const float fill = kLogits ? ER_LOGIT_FILL : 0.f;
   typename Load8<T>::Raw rp = Load8<T>::load(trow, v0, V, vec, fill), rq = rp;
   if (use_q) rq = Load8<T>::load(drow, v0, V, vec, fill);
   weights8_raw<T, kLogits>(rp, rq, scale, st, sd, use_q, w);
@@ -397,7 +400,7 @@ __device__ void draw_segment_sums(const T* trow, const T* drow, int V, bool vec,
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int nloc = cx.seg_hi - cx.seg_lo;
   constexpr int NB = Load8<T>::kBatch;
-  const float fill = kLogits ? kNegInf : 0.f;
+  const float fill = kLogits ? ER_LOGIT_FILL : 0.f;
   for (int s0 = warp; s0 < nloc; s0 += NB * kWarps) {
     typename Load8<T>::Raw rp[NB], rq[NB];
 #pragma unroll
@@ -753,7 +756,7 @@ __device__ __forceinline__ void consume_row_stats(const unsigned char* ring, Sha
         r[j] = Accum<T>::neg_inf();
         if (sg < nloc && v0 < V) {
           r[j] = *reinterpret_cast<const Raw*>(stage + off[j]);
-          clip_tail(r[j], v0, V, kNegInf);
+          clip_tail(r[j], v0, V, ER_LOGIT_FILL);
         }
       }
     }
@@ -784,10 +787,10 @@ __device__ __forceinline__ void consume_segment_sums(const unsigned char* ring, 
       if (v0 < V) {
         const size_t o = (size_t)warp * R::kSegBytes + (size_t)lane * kPerThread * sizeof(T);
         typename Load8<T>::Raw rp = *reinterpret_cast<const typename Load8<T>::Raw*>(stage + o), rq = rp;
-        clip_tail(rp, v0, V, kNegInf);
+        clip_tail(rp, v0, V, ER_LOGIT_FILL);
         if (use_q) {
           rq = *reinterpret_cast<const typename Load8<T>::Raw*>(stage + R::kStageBytes / 2 + o);
-          clip_tail(rq, v0, V, kNegInf);
+          clip_tail(rq, v0, V, ER_LOGIT_FILL);
         }
         float w[8];
         weights8_raw<T, true>(rp, rq, scale, st, sd, use_q, w);

@@ -169,10 +169,15 @@ def test_config2_maximum_batch_256_gamma_8():
     _check_against_oracle(tgt, drf, toks, ua, us, acc, out, rows=rows)
 
 
-def test_masked_logits_minus_infinity():
+@pytest.mark.parametrize("dtype", [torch.float32, torch.bfloat16])
+@pytest.mark.parametrize("V", [20011, 20012, 20016, 5001])
+def test_masked_logits_minus_infinity(V, dtype):
     # logits after top-k style masking: everything outside the top 50 of the TARGET row is -inf in both rows (also whole
-    # 8-element chunks and whole tiles); the kernel must not produce NaN statistics
-    B, gamma, V = 6, 3, 20011
+    # 8-element chunks, whole segments and the ragged tail chunk, whose positions beyond V are filled by the kernel);
+    # the kernel must not produce NaN / inf statistics (a finite fill value once became a lane's softmax
+    # reference there).  V = 20011 / 5001: scalar loads; 20012: fp32 rows through the ring with a clipped tail; 20016:
+    # both dtypes through the ring
+    B, gamma = 6, 3
     lt, ld = I.verify_logits_f32(B, gamma, V, 4242, draft_noise=0.5)
     for b in range(B):
         for i in range(gamma + 1):
@@ -182,11 +187,15 @@ def test_masked_logits_minus_infinity():
             lt[b, i, m] = -np.inf
             if i < gamma:
                 ld[b, i, m] = -np.inf
+    lt = torch.from_numpy(lt).to(dtype).float().numpy()
+    ld = torch.from_numpy(ld).to(dtype).float().numpy()
     toks = I.sample_draft_tokens(_softmax(ld), 4243)
-    acc, out, _ = _run_and_check(lt, ld, toks, I.uniforms((B, gamma), 4244), I.uniforms((B,), 4245), True, torch.float32)
-    assert np.all(out[np.arange(B), acc] >= 0)
-    for b in range(B):
-        assert np.isfinite(lt[b, acc[b], out[b, acc[b]]])        # the drawn token is never a masked one
+    for T in (1.0, 0.6):
+        acc, out, _ = _run_and_check(lt, ld, toks, I.uniforms((B, gamma), 4244), I.uniforms((B,), 4245), True, dtype,
+                                     temperature=T)
+        assert np.all(out[np.arange(B), acc] >= 0)
+        for b in range(B):
+            assert np.isfinite(lt[b, acc[b], out[b, acc[b]]])        # the drawn token is never a masked one
 
 
 def test_temperature():
