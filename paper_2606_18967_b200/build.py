@@ -16,7 +16,7 @@ INCLUDE = os.path.join(os.path.dirname(PKG_DIR), "include")
 LIB_PATH = os.path.join(PKG_DIR, "liber_b200.so")
 DEV_LIB_PATH = os.path.join(PKG_DIR, "liber_b200_dev.so")
 SOURCES = ["er_api.cu", "er_host.cu", "quantize_pack.cu", "spec_verify.cu", "w4a16_gemm_simt.cu", "w4a16_gemm.cu",
-           "w4a16_gemm_small.cu", "w4a16_gemm_large.cu", "bf16_gemm.cu", "sd_policy.cu", "quantize_pack8.cu"]
+           "w4a16_gemm_small.cu", "w4a16_gemm_wide.cu", "w4a16_gemm_large.cu", "bf16_gemm.cu", "sd_policy.cu", "quantize_pack8.cu"]
 NVCC_FLAGS = ["-std=c++17", "-O3", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC]
 

@@ -585,7 +585,7 @@ w4a16_gemm_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
 namespace er {
 
 #ifdef ER_DEV
-Tuning g_tune = {1, 1, 1, 0, 1, 0};
+Tuning g_tune = {1, 1, 1, 0, 1, 0, 1, 0};
 #endif
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -626,6 +626,25 @@ int max_active_clusters16(int c);
 
 int mpad_of(int64_t M) { return M <= 16 ? 16 : (M <= 32 ? 32 : 64); }
 
+// M > 64: which kernel (64-row chunks here, or the 128-row kernel of w4a16_gemm_wide.cu) and which partition (whole tiles,
+// or stream-K ranges whose partial tiles go through the workspace).  Estimated microseconds from measured constants
+// (profiles/r02_gemm.md section 10): 0.40 / 0.54 us per 128-k group and SM for a tile of 64 / 128 batch rows, 22 / 14 us for
+// the partial-tile traffic and reduction of a stream-K plan (partials of 32 / 64 KB written and re-read at the end of the
+// launch, by all CTAs at once).
+struct PlanAbove64 { bool wide, whole_wide, whole_narrow; };
+PlanAbove64 plan_above_64(int64_t M, int64_t N, int64_t K, bool planes) {
+  const Tuning& tn = er::g_tune;
+  const long long sms = er::sm_count(), G = K / ER_GROUP, ntiles = N / kTileN;
+  const long long tn_ = ntiles * ((M + 63) / 64), tw_ = ntiles * ((M + 127) / 128);
+  const double whole_n = (double)((tn_ + sms - 1) / sms) * G * 0.40, sk_n = (double)((tn_ * G + sms - 1) / sms) * 0.40 + 22.0;
+  const double whole_w = (double)((tw_ + sms - 1) / sms) * G * 0.54, sk_w = (double)((tw_ * G + sms - 1) / sms) * 0.54 + 14.0;
+  PlanAbove64 r;
+  r.wide = !planes && tn.wide != 0 && (tn.wide == 2 || fmin(whole_w, sk_w) < fmin(whole_n, sk_n));
+  r.whole_wide = tn.units == 1 || (tn.units == 0 && whole_w <= sk_w);
+  r.whole_narrow = tn.units == 1 || (tn.units == 0 && whole_n <= sk_n);
+  return r;
+}
+
 Plan make_plan(int64_t M, int64_t N, int64_t K) {
   const Tuning& tn = er::g_tune;
   Plan pl;
@@ -638,13 +657,9 @@ Plan make_plan(int64_t M, int64_t N, int64_t K) {
   pl.unit_groups = (pl.tiles <= ER_GEMM_COUNTER_BYTES / 4) ? 1 : pl.G;
   int ctas = er::sm_count();
   if (tn.force_ctas > 0 && tn.force_ctas < ctas) ctas = tn.force_ctas;
-  // M > 64 (several chunks of 64 batch rows, every (chunk, weight tile) a tile of its own): whole tiles when they keep
-  // the CTAs about as busy as stream-K ranges would -- a partial tile is 32 KB there
-  if (pl.mchunks > 1 && tn.force_ctas == 0) {
-    const long long whole = (long long)((pl.tiles + ctas - 1) / ctas) * pl.G;
-    const long long sk = ((long long)pl.tiles * pl.G + ctas - 1) / ctas;
-    if (whole * 100 <= sk * 115) pl.unit_groups = pl.G;
-  }
+  // M > 64 (several chunks of 64 batch rows, every (chunk, weight tile) a tile of its own): whole tiles where the cost
+  // model prefers them to stream-K ranges (plan_above_64)
+  if (M > 64 && tn.force_ctas == 0 && plan_above_64(M, N, K, true).whole_narrow) pl.unit_groups = pl.G;
   pl.units = (long long)pl.tiles * pl.G / pl.unit_groups;
   if ((long long)ctas > pl.units) ctas = (int)pl.units;
   pl.ctas = ctas;
@@ -751,6 +766,8 @@ int er_dev_gemm_tuning(int key, int value) {
   if (key == 5 && (value == 0 || value == 1)) { er::g_tune.cluster = value; return ER_OK; }
   if (key == 6 && (value == 0 || value == 1)) { er::g_tune.small_mma = value; return ER_OK; }
   if (key == 7 && value >= 0 && value <= 2) { er::g_tune.large = value; return ER_OK; }
+  if (key == 8 && value >= 0 && value <= 2) { er::g_tune.wide = value; return ER_OK; }
+  if (key == 9 && value >= 0 && value <= 2) { er::g_tune.units = value; return ER_OK; }
   return ER_ERR_SHAPE;
 }
 #endif
@@ -758,7 +775,11 @@ int er_dev_gemm_tuning(int key, int value) {
 
 size_t er_gemm_workspace_bytes(int64_t M, int64_t N, int64_t K) {
   if (M < 1 || N < kTileN || N % kTileN != 0 || K < ER_GROUP || K % ER_GROUP != 0) return 0;
-  const size_t exact = workspace_for(mpad_of(M));
+  size_t exact = workspace_for(mpad_of(M));
+  if (M > 64) {   // the 128-row kernel's partial tiles (w4a16_gemm_wide.cu)
+    const size_t wide = er::wide_workspace_bytes();
+    if (wide > exact) exact = wide;
+  }
 #ifdef ER_DEV   // the development library can switch to the pre-scaled large-batch kernel (w4a16_gemm_large.cu)
   const size_t large = M > 16 ? er::large_workspace_bytes(M, N, K) : 0;
   return exact > large ? exact : large;
@@ -812,6 +833,11 @@ static int gemm_impl(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems
   if (!planes && M > 16 && (er::g_tune.large == 2 || (er::g_tune.large == 1 && er::large_preferred(M, N, K))))
     return er::launch_large(x_bf16, M, N, K, ldx_elems, gp, s);
 #endif
+  // M > 64: a batch tile of 128 rows, the weights converted once per tile (w4a16_gemm_wide.cu)
+  if (M > 64) {
+    const PlanAbove64 pa = plan_above_64(M, N, K, planes != 0);
+    if (pa.wide) return er::launch_wide(x_bf16, M, N, K, ldx_elems, gp, pa.whole_wide, s);
+  }
   // M <= 8 on a plan without a cluster (the large-N linears: gate/up): the warp-level-MMA kernel streams them faster
   // (w4a16_gemm_small.cu; measured in profiles/r02_gemm.md)
   if (!planes && M <= 8 && pl.cluster == 1 && er::g_tune.small_mma) return er::launch_small(x_bf16, M, K, ldx_elems, gp, pl, s);

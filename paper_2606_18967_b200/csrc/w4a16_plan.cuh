@@ -73,11 +73,14 @@ struct Tuning {
   int small_mma;    // M <= 8 without a cluster through the warp-level-MMA kernel (0: through the tcgen05 kernel)
   int large;        // 1: the pre-scaled large-batch kernel where it is preferred (M > 64, whole tiles); 0: never;
                     // 2: for every M > 16 (tests)
+  int wide;         // M > 64 through the 128-row kernel (w4a16_gemm_wide.cu): 1 where the plan prefers it, 2 always;
+                    // 0: in chunks of 64 rows (w4a16_gemm.cu)
+  int units;        // M > 64: 0 = plan's choice, 1 = whole tiles, 2 = stream-K ranges (tests / measurements)
 };
 #ifdef ER_DEV
 extern Tuning g_tune;
 #else
-constexpr Tuning g_tune = {1, 1, 1, 0, 1, 0};
+constexpr Tuning g_tune = {1, 1, 1, 0, 1, 0, 1, 0};
 #endif
 
 // 2-D row-major tensor [rows][cols] of elements, row pitch in bytes, box [box_rows][box_cols].
@@ -87,7 +90,11 @@ bool make_map_2d(CUtensorMap* map, CUtensorMapDataType dt, const void* base, uin
 // M <= 8, no cluster: w4a16_gemm_small.cu
 int launch_small(const void* x, int64_t M, int64_t K, int64_t ldx, GemmParams gp, const Plan& pl, cudaStream_t stream);
 
-// M > 16: w4a16_gemm_large.cu
+// M > 64: w4a16_gemm_wide.cu
+size_t wide_workspace_bytes();
+int launch_wide(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, GemmParams gp, bool whole, cudaStream_t stream);
+
+// M > 16, development library only: w4a16_gemm_large.cu
 int large_mpad_of(int64_t M);
 size_t large_workspace_bytes(int64_t M, int64_t N, int64_t K);
 bool large_preferred(int64_t M, int64_t N, int64_t K);

@@ -133,7 +133,7 @@ def dev_library():
     try:
         yield lib
     finally:
-        for key, value in ((1, 0), (3, 1), (4, 1), (5, 1), (6, 1), (7, 0)):
+        for key, value in ((1, 0), (3, 1), (4, 1), (5, 1), (6, 1), (7, 0), (8, 1), (9, 0)):
             lib.er_dev_gemm_tuning(key, value)
         lib.er_dev_verify_cluster(0)
         lib.er_dev_verify_cluster(16)

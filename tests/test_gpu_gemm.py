@@ -404,10 +404,12 @@ def test_partition_modes_at_m_17_to_32(mode, M):
         torch.cuda.synchronize()
         assert torch.equal(y1, y2)
 
+@pytest.mark.parametrize("wide", [0, 2])
 @pytest.mark.parametrize("M", [65, 130, 200, 256, 300])
-def test_exact_kernel_above_64_rows_every_plan(M):
-    # M > 64 runs in chunks of 64 batch rows, (chunk, weight tile) = a tile of its own: whole tiles (the automatic plan
-    # here), stream-K ranges whose partial tiles go through the workspace (forced CTA counts), the last chunk ragged;
+def test_exact_kernels_above_64_rows_every_plan(M, wide):
+    # M > 64 runs either in chunks of 64 batch rows (w4a16_gemm.cu, dev key 8 = 0) or in tiles of 128 batch rows
+    # (w4a16_gemm_wide.cu, key 8 = 2: always); (chunk, weight tile) = a tile of its own: whole tiles (key 9 = 1), stream-K
+    # ranges whose partial tiles go through the workspace (key 9 = 2, and forced CTA counts), the last chunk ragged;
     # integer probe: bit-exact against the oracle, i.e. no rounding of q * s at any M
     N, K = 1024, 1152
     codes = I.random_codes(N, K, 31)
@@ -422,11 +424,14 @@ def test_exact_kernel_above_64_rows_every_plan(M):
     xg = I.activation_bf16(M, K, I.seed_of("exact64", M), device=DEV)
     ref2 = O.w4a16_gemm(I.as_u16(xg), qw2.cpu().numpy().view(np.uint32), su2)
     with er.dev_library() as lib:
-        for ctas in (0, 5, 37, 148):
-            assert lib.er_dev_gemm_tuning(1, ctas) == 0
+        assert lib.er_dev_gemm_tuning(8, wide) == 0
+        for ctas, units in ((0, 1), (0, 2), (5, 0), (37, 0), (148, 0)):
+            assert lib.er_dev_gemm_tuning(1, ctas) == 0 and lib.er_dev_gemm_tuning(9, units) == 0
             y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
             y2 = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
-            assert np.array_equal(y.cpu().numpy().astype(np.float64), ref), (M, ctas)
+            yb = er.w4a16_gemm(x, qw, sc, out_dtype=torch.bfloat16)
+            assert np.array_equal(y.cpu().numpy().astype(np.float64), ref), (M, ctas, units)
             assert torch.equal(y, y2)
+            assert np.array_equal(I.as_u16(yb), O.f32_to_bf16_rne(y.cpu().numpy()))
             yg = er.w4a16_gemm(xg, qw2, sc2, out_dtype=torch.float32).cpu().numpy().astype(np.float64)
-            assert np.abs(yg - ref2).max() <= 1e-5 * np.sqrt(np.mean(ref2 ** 2)) + 1e-6, (M, ctas)   # fp32 summation only
+            assert np.abs(yg - ref2).max() <= 1e-5 * np.sqrt(np.mean(ref2 ** 2)) + 1e-6, (M, ctas, units)   # fp32 summation only
