@@ -196,13 +196,17 @@ w4a16_wide_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
     int it = 0;
     int pend_tile[2] = {-1, -1};
 
-    auto read_back = [&]() {
+    // scale-accumulate of the oldest group in flight, in two halves so that other work can sit between the tcgen05.ld and
+    // its use: read_back_issue() waits for the group's MMAs and starts the loads, read_back_finish() consumes them
+    uint32_t d[kCW];
+    auto read_back_issue = [&]() {
       mbar_wait(&done[rbuf], (pd >> rbuf) & 1);
       pd ^= 1u << rbuf;
       tc_fence_after();
-      uint32_t d[kCW];
       ERW_TMEM_LD16(d_t + rbuf * kMP, d, 0);
       ERW_TMEM_LD16(d_t + rbuf * kMP + 16, d, 16);
+    };
+    auto read_back_finish = [&]() {
       asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
 #pragma unroll
       for (int m = 0; m < kCW; ++m) acc[m] = fmaf(sc_old, __uint_as_float(d[m]), acc[m]);
@@ -222,15 +226,19 @@ w4a16_wide_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
       for (; it < it_end; ++it) {
         mbar_wait(&full[s], ph);
         const uint32_t st = s * kStageBytes;
-        if (npend == 2) read_back();         // the group before last: frees the A buffer and accumulator written next
         const uint4 pk = lds128(st + w_addr);
         const uint32_t sc16 = lds_u16(st + sc_addr);
+        // the group before last frees the A buffer and the accumulator written next; its TENSOR-MEMORY loads are in flight
+        // while this group is converted, and their use hides the latency of the A operand's store
+        const bool drain = (npend == 2);
+        if (drain) read_back_issue();
         uint32_t a[16];
         dequant_word(pk.x, a + 0);
         dequant_word(pk.y, a + 4);
         dequant_word(pk.z, a + 8);
         dequant_word(pk.w, a + 12);
         ERW_TMEM_ST16(a_t + wbuf * 64, a);
+        if (drain) read_back_finish();
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
         tc_fence_before();
         __syncwarp();
@@ -241,7 +249,7 @@ w4a16_wide_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
         wbuf ^= 1;
         if (++s == S) { s = 0; ph ^= 1; }
       }
-      while (npend > 0) read_back();
+      while (npend > 0) { read_back_issue(); read_back_finish(); }
 
       // ---- output: a whole tile is stored directly; a partial one goes to the workspace as fp32 ----
       const int n = (tile % p.ntiles) * kTileN + row, m0 = (tile / p.ntiles) * kMP + part * kCW;
