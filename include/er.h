@@ -115,12 +115,12 @@ int er_quantize_pack_batched(const er_linear_desc* descs, int count, int group, 
  *            row stride ldy_elems; rows >= M are never written
  *   workspace  caller-provided, >= er_gemm_workspace_bytes(M,N,K), 16-byte aligned, counters zeroed once
  *            (N/128) * (K/128) * ceil(M / 64) must stay below 2^31 (else ER_ERR_SHAPE)
- * Arithmetic (two kernels, chosen from M and the work plan), the same at every M:
+ * Arithmetic (three kernels, chosen from M and the work plan), the same at every M:
  *   stored nibbles u = q + 8 are widened exactly to bf16 (as 128 + u) and contracted with X on the tensor cores with fp32
  *   accumulation per 128-k group; the 136 * sum_k x[m][k] the offset adds is removed on that fp32 sum (M <= 16: through a
  *   constant operand tile, or with the x sums computed beside the contraction) or on the widened nibbles (M > 16: one
  *   packed fma, exact), so the sum holds sum_k x * q up to fp32 rounding; each group's sum is multiplied by its fp32 scale
- *   and added in fp32: q * s is NEVER rounded.  M > 64 runs in chunks of 64 batch rows.
+ *   and added in fp32: q * s is NEVER rounded.  M > 64 runs in tiles of 128 or chunks of 64 batch rows (chosen per problem).
  *   Split-K partials are reduced in ascending CTA order, or inside a thread-block cluster in rank order; every kernel is
  *   deterministic (identical inputs, identical bits; no floating-point atomics).
  * Launch: one persistent kernel, launched with programmatic stream serialization; it touches no global memory before
