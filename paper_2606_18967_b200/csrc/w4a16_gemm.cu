@@ -631,15 +631,20 @@ int mpad_of(int64_t M) { return M <= 16 ? 16 : (M <= 32 ? 32 : 64); }
 // (profiles/r02_gemm.md section 10): 0.40 / 0.54 us per 128-k group and SM for a tile of 64 / 128 batch rows, 22 / 14 us for
 // the partial-tile traffic and reduction of a stream-K plan (partials of 32 / 64 KB written and re-read at the end of the
 // launch, by all CTAs at once).
-struct PlanAbove64 { bool wide, whole_wide, whole_narrow; };
+struct PlanAbove64 { bool wide, whole_wide, whole_narrow; int split_wide; };
 PlanAbove64 plan_above_64(int64_t M, int64_t N, int64_t K, bool planes) {
   const Tuning& tn = er::g_tune;
   const long long sms = er::sm_count(), G = K / ER_GROUP, ntiles = N / kTileN;
   const long long tn_ = ntiles * ((M + 63) / 64), tw_ = ntiles * ((M + 127) / 128);
   const double whole_n = (double)((tn_ + sms - 1) / sms) * G * 0.40, sk_n = (double)((tn_ * G + sms - 1) / sms) * 0.40 + 22.0;
   const double whole_w = (double)((tw_ + sms - 1) / sms) * G * 0.54, sk_w = (double)((tw_ * G + sms - 1) / sms) * 0.54 + 14.0;
+  // wide kernel, tile split: k parts per tile, one partial tile per CTA instead of two
+  const long long ks = tw_ > 0 ? sms / tw_ : 0;
+  const double split_w = (ks >= 2 && ks <= G && tn.split) ? (double)((G + ks - 1) / ks) * 0.54 + 14.0 * (double)(tw_ * ks) / (2.0 * sms)
+                                                          : 1e30;
   PlanAbove64 r;
-  r.wide = !planes && tn.wide != 0 && (tn.wide == 2 || fmin(whole_w, sk_w) < fmin(whole_n, sk_n));
+  r.split_wide = (tn.units == 0 && split_w < fmin(whole_w, sk_w)) ? (int)ks : 0;
+  r.wide = !planes && tn.wide != 0 && (tn.wide == 2 || fmin(fmin(whole_w, sk_w), split_w) < fmin(whole_n, sk_n));
   r.whole_wide = tn.units == 1 || (tn.units == 0 && whole_w <= sk_w);
   r.whole_narrow = tn.units == 1 || (tn.units == 0 && whole_n <= sk_n);
   return r;
@@ -836,7 +841,7 @@ static int gemm_impl(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems
   // M > 64: a batch tile of 128 rows, the weights converted once per tile (w4a16_gemm_wide.cu)
   if (M > 64) {
     const PlanAbove64 pa = plan_above_64(M, N, K, planes != 0);
-    if (pa.wide) return er::launch_wide(x_bf16, M, N, K, ldx_elems, gp, pa.whole_wide, s);
+    if (pa.wide) return er::launch_wide(x_bf16, M, N, K, ldx_elems, gp, pa.whole_wide, pa.split_wide, s);
   }
   // M <= 8 on a plan without a cluster (the large-N linears: gate/up): the warp-level-MMA kernel streams them faster
   // (w4a16_gemm_small.cu; measured in profiles/r02_gemm.md)

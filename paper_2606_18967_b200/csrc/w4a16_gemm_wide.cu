@@ -350,7 +350,8 @@ namespace er {
 size_t wide_workspace_bytes() { return ER_GEMM_COUNTER_BYTES + (size_t)sm_count() * 2 * kMP * kTileN * sizeof(float); }
 
 // M > 64: `gp` arrives with the problem, the output and the workspace filled in; the partition is made here.
-int launch_wide(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, GemmParams gp, bool whole, cudaStream_t stream) {
+int launch_wide(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, GemmParams gp, bool whole, int split,
+                cudaStream_t stream) {
   const int mchunks = (int)((M + kMP - 1) / kMP), ntiles = (int)(N / kTileN), G = (int)(K / ER_GROUP);
   const long long tiles = (long long)ntiles * mchunks;
   if (tiles * G >= (1ll << 31)) return ER_ERR_SHAPE;
@@ -365,6 +366,11 @@ int launch_wide(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, Gem
   gp.G = G; gp.ntiles = ntiles; gp.mchunks = mchunks; gp.tiles = (int)tiles; gp.unit_groups = unit_groups;
   gp.units = (int)units; gp.uq = (int)(units / ctas); gp.ur = (int)(units % ctas);
   gp.split = 0; gp.cluster = 1; gp.planes = 0;
+  if (split >= 2 && unit_groups == 1 && g_tune.force_ctas == 0 && tiles * split <= sm_count()) {
+    // tile split: CTA c owns part c % split of tile c / split (w4a16_plan.cuh): one segment and one partial tile per CTA
+    gp.split = split; gp.uq = G; gp.ur = 0;
+    ctas = (int)(tiles * split);
+  }
   CUtensorMap mx;
   if (!make_map_2d(&mx, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, x, (uint64_t)M, (uint64_t)K, (uint64_t)ldx * 2, (uint32_t)kMP, 64,
                    CU_TENSOR_MAP_SWIZZLE_128B)) {

@@ -92,7 +92,8 @@ int launch_small(const void* x, int64_t M, int64_t K, int64_t ldx, GemmParams gp
 
 // M > 64: w4a16_gemm_wide.cu
 size_t wide_workspace_bytes();
-int launch_wide(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, GemmParams gp, bool whole, cudaStream_t stream);
+int launch_wide(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, GemmParams gp, bool whole, int split,
+                cudaStream_t stream);
 
 // M > 16, development library only: w4a16_gemm_large.cu
 int large_mpad_of(int64_t M);

@@ -435,3 +435,22 @@ def test_exact_kernels_above_64_rows_every_plan(M, wide):
             assert np.array_equal(I.as_u16(yb), O.f32_to_bf16_rne(y.cpu().numpy()))
             yg = er.w4a16_gemm(xg, qw2, sc2, out_dtype=torch.float32).cpu().numpy().astype(np.float64)
             assert np.abs(yg - ref2).max() <= 1e-5 * np.sqrt(np.mean(ref2 ** 2)) + 1e-6, (M, ctas, units)   # fp32 summation only
+
+
+@pytest.mark.parametrize("M", [65, 128, 200])
+def test_above_64_rows_long_k_few_tiles_automatic_plan(M):
+    # the shape class of `down` (few weight tiles, long K): the cost model picks the 128-row kernel with a TILE SPLIT (k
+    # CTAs per tile, one partial tile each, ticket reduction); integer probe: bit-exact, deterministic
+    N, K = 256, 18944
+    codes = I.random_codes(N, K, 41)
+    su = np.full((K // 128, N), 0x3F80, dtype=np.uint16)
+    su[1::2] = 0x4000
+    qw, sc = _dev_weights(codes, su)
+    rng = np.random.default_rng(M)
+    x = torch.from_numpy(rng.integers(-1, 3, size=(M, K)).astype(np.float32)).to(DEV).to(torch.bfloat16)
+    ref = O.w4a16_gemm(I.as_u16(x), qw.cpu().numpy().view(np.uint32), su)
+    y = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
+    y2 = er.w4a16_gemm(x, qw, sc, out_dtype=torch.float32)
+    torch.cuda.synchronize()
+    assert np.array_equal(y.cpu().numpy().astype(np.float64), ref)
+    assert torch.equal(y, y2)
