@@ -638,9 +638,10 @@ PlanAbove64 plan_above_64(int64_t M, int64_t N, int64_t K, bool planes) {
   const long long tn_ = ntiles * ((M + 63) / 64), tw_ = ntiles * ((M + 127) / 128);
   const double whole_n = (double)((tn_ + sms - 1) / sms) * G * 0.40, sk_n = (double)((tn_ * G + sms - 1) / sms) * 0.40 + 22.0;
   const double whole_w = (double)((tw_ + sms - 1) / sms) * G * 0.54, sk_w = (double)((tw_ * G + sms - 1) / sms) * 0.54 + 14.0;
-  // wide kernel, tile split: k parts per tile, one partial tile per CTA instead of two
+  // wide kernel, tile split: k parts per tile, one partial tile per CTA instead of two (measured: ~6 us + the share of the
+  // stream-K figure that the number of partial tiles makes up)
   const long long ks = tw_ > 0 ? sms / tw_ : 0;
-  const double split_w = (ks >= 2 && ks <= G && tn.split) ? (double)((G + ks - 1) / ks) * 0.54 + 14.0 * (double)(tw_ * ks) / (2.0 * sms)
+  const double split_w = (ks >= 2 && ks <= G && tn.split) ? (double)((G + ks - 1) / ks) * 0.54 + 6.0 + 14.0 * (double)(tw_ * ks) / (2.0 * sms)
                                                           : 1e30;
   PlanAbove64 r;
   r.split_wide = (tn.units == 0 && split_w < fmin(whole_w, sk_w)) ? (int)ks : 0;
