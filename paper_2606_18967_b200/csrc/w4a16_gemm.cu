@@ -645,7 +645,8 @@ PlanAbove64 plan_above_64(int64_t M, int64_t N, int64_t K, bool planes) {
                                                           : 1e30;
   PlanAbove64 r;
   r.split_wide = (tn.units == 0 && split_w < fmin(whole_w, sk_w)) ? (int)ks : 0;
-  r.wide = !planes && tn.wide != 0 && (tn.wide == 2 || fmin(fmin(whole_w, sk_w), split_w) < fmin(whole_n, sk_n));
+  (void)planes;   // the two-plane W8 matrix is a W4 matrix with 2 K columns for this purpose
+  r.wide = tn.wide != 0 && (tn.wide == 2 || fmin(fmin(whole_w, sk_w), split_w) < fmin(whole_n, sk_n));
   r.whole_wide = tn.units == 1 || (tn.units == 0 && whole_w <= sk_w);
   r.whole_narrow = tn.units == 1 || (tn.units == 0 && whole_n <= sk_n);
   return r;
@@ -841,8 +842,8 @@ static int gemm_impl(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_elems
 #endif
   // M > 64: a batch tile of 128 rows, the weights converted once per tile (w4a16_gemm_wide.cu)
   if (M > 64) {
-    const PlanAbove64 pa = plan_above_64(M, N, K, planes != 0);
-    if (pa.wide) return er::launch_wide(x_bf16, M, N, K, ldx_elems, gp, pa.whole_wide, pa.split_wide, s);
+    const PlanAbove64 pa = plan_above_64(M, N, Kw, planes != 0);
+    if (pa.wide) return er::launch_wide(x_bf16, M, N, Kw, ldx_elems, gp, pa.whole_wide, pa.split_wide, s);
   }
   // M <= 8 on a plan without a cluster (the large-N linears: gate/up): the warp-level-MMA kernel streams them faster
   // (w4a16_gemm_small.cu; measured in profiles/r02_gemm.md)

@@ -56,12 +56,12 @@ static_assert(kSmem <= kSmemLimit, "shared memory");
 
 // One packed word -> 4 registers of bf16 pairs (q, q'): (w >> 4t) & 0x000F000F | 0x43004300 = (128 + u, 128 + u'), then
 // one packed fma removes the 136 exactly (u = q + 8).
-__device__ __forceinline__ void dequant_word(uint32_t w, uint32_t* a) {
+__device__ __forceinline__ void dequant_word(uint32_t w, uint32_t* a, uint32_t off2) {
 #pragma unroll
   for (int t = 0; t < 4; ++t) {
     uint32_t v;
     asm("lop3.b32 %0, %1, %2, %3, 0xEA;" : "=r"(v) : "r"(w >> (4 * t)), "r"(0x000F000Fu), "r"(0x43004300u));
-    asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(a[t]) : "r"(v), "r"(0x3F803F80u), "r"(0xC308C308u));
+    asm("fma.rn.bf16x2 %0, %1, %2, %3;" : "=r"(a[t]) : "r"(v), "r"(0x3F803F80u), "r"(off2));
   }
 }
 
@@ -79,6 +79,9 @@ __device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("ba
 
 __device__ __forceinline__ void named_bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
+// kPlanes: the two-plane W8 instantiation (er_w8a16_gemm; w4a16_gemm.cu): groups 2g, 2g + 1 of the packed matrix contract
+// the same 128 columns of X; the high-nibble plane (even groups; G is even) takes -136 per widened nibble, the low one -128.
+template <bool kPlanes>
 __global__ void __launch_bounds__(kThreads, 1)
 w4a16_wide_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p) {
   constexpr int S = kStages;
@@ -135,8 +138,9 @@ w4a16_wide_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
         uint8_t* st = smem + s * kStageBytes;
         mbar_arrive_expect_tx(&full[s], kTxBytes);
         bulk_load_1d(st, p.qweight + ((size_t)tn * p.G + g) * kWBytes, kWBytes, &full[s], kEvictFirst);
-        tma_load_2d(st + kWBytes, &map_x, &full[s], g * 128, mc * kMP, kEvictLast);
-        tma_load_2d(st + kWBytes + kMP * 128, &map_x, &full[s], g * 128 + 64, mc * kMP, kEvictLast);
+        const int xk = (g >> (kPlanes ? 1 : 0)) * 128;
+        tma_load_2d(st + kWBytes, &map_x, &full[s], xk, mc * kMP, kEvictLast);
+        tma_load_2d(st + kWBytes + kMP * 128, &map_x, &full[s], xk + 64, mc * kMP, kEvictLast);
         bulk_load_1d(st + kWBytes + kXBytes, p.scales + ((size_t)g * p.N + tn * kTileN) * 2, kScaleBytes, &full[s],
                      kEvictFirst);
       }
@@ -232,11 +236,12 @@ w4a16_wide_kernel(const __grid_constant__ CUtensorMap map_x, const GemmParams p)
         // while this group is converted, and their use hides the latency of the A operand's store
         const bool drain = (npend == 2);
         if (drain) read_back_issue();
+        const uint32_t off2 = (kPlanes && ((gb + it) & 1)) ? 0xC300C300u : 0xC308C308u;   // (-128, -128) : (-136, -136)
         uint32_t a[16];
-        dequant_word(pk.x, a + 0);
-        dequant_word(pk.y, a + 4);
-        dequant_word(pk.z, a + 8);
-        dequant_word(pk.w, a + 12);
+        dequant_word(pk.x, a + 0, off2);
+        dequant_word(pk.y, a + 4, off2);
+        dequant_word(pk.z, a + 8, off2);
+        dequant_word(pk.w, a + 12, off2);
         ERW_TMEM_ST16(a_t + wbuf * 64, a);
         if (drain) read_back_finish();
         asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
@@ -351,7 +356,8 @@ size_t wide_workspace_bytes() { return ER_GEMM_COUNTER_BYTES + (size_t)sm_count(
 
 // M > 64: `gp` arrives with the problem, the output and the workspace filled in; the partition is made here.
 int launch_wide(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, GemmParams gp, bool whole, int split,
-                cudaStream_t stream) {
+                cudaStream_t stream) {   // K = columns of the PACKED matrix (2 x the columns of X for two-plane W8: gp.planes)
+  const bool planes = gp.planes != 0;
   const int mchunks = (int)((M + kMP - 1) / kMP), ntiles = (int)(N / kTileN), G = (int)(K / ER_GROUP);
   const long long tiles = (long long)ntiles * mchunks;
   if (tiles * G >= (1ll << 31)) return ER_ERR_SHAPE;
@@ -365,14 +371,14 @@ int launch_wide(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, Gem
   if ((long long)ctas > units) ctas = (int)units;
   gp.G = G; gp.ntiles = ntiles; gp.mchunks = mchunks; gp.tiles = (int)tiles; gp.unit_groups = unit_groups;
   gp.units = (int)units; gp.uq = (int)(units / ctas); gp.ur = (int)(units % ctas);
-  gp.split = 0; gp.cluster = 1; gp.planes = 0;
+  gp.split = 0; gp.cluster = 1;
   if (split >= 2 && unit_groups == 1 && g_tune.force_ctas == 0 && tiles * split <= sm_count()) {
     // tile split: CTA c owns part c % split of tile c / split (w4a16_plan.cuh): one segment and one partial tile per CTA
     gp.split = split; gp.uq = G; gp.ur = 0;
     ctas = (int)(tiles * split);
   }
   CUtensorMap mx;
-  if (!make_map_2d(&mx, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, x, (uint64_t)M, (uint64_t)K, (uint64_t)ldx * 2, (uint32_t)kMP, 64,
+  if (!make_map_2d(&mx, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, x, (uint64_t)M, (uint64_t)(planes ? K / 2 : K), (uint64_t)ldx * 2, (uint32_t)kMP, 64,
                    CU_TENSOR_MAP_SWIZZLE_128B)) {
     set_last_cuda_error((int)cudaErrorInvalidValue);
     return ER_ERR_CUDA;
@@ -380,7 +386,8 @@ int launch_wide(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, Gem
   static bool attr_set[kMaxDevices] = {};
   const int dev = current_device();
   if (dev < 0 || dev >= kMaxDevices || !attr_set[dev]) {
-    ER_CUDA_TRY(cudaFuncSetAttribute(w4a16_wide_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
+    ER_CUDA_TRY(cudaFuncSetAttribute(w4a16_wide_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
+    ER_CUDA_TRY(cudaFuncSetAttribute(w4a16_wide_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmem));
     if (dev >= 0 && dev < kMaxDevices) attr_set[dev] = true;
   }
   cudaLaunchConfig_t cfg = {};
@@ -393,7 +400,8 @@ int launch_wide(const void* x, int64_t M, int64_t N, int64_t K, int64_t ldx, Gem
   attr[0].val.programmaticStreamSerializationAllowed = g_tune.pdl;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
-  ER_CUDA_TRY(cudaLaunchKernelEx(&cfg, w4a16_wide_kernel, mx, gp));
+  if (planes) ER_CUDA_TRY(cudaLaunchKernelEx(&cfg, w4a16_wide_kernel<true>, mx, gp));
+  else ER_CUDA_TRY(cudaLaunchKernelEx(&cfg, w4a16_wide_kernel<false>, mx, gp));
   return ER_OK;
 }
 

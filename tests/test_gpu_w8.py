@@ -72,7 +72,7 @@ def test_gemm_every_batch_size(M):
 
 
 @pytest.mark.parametrize("K", [3584, 18944])
-@pytest.mark.parametrize("M", [1, 16, 64])
+@pytest.mark.parametrize("M", [1, 16, 64, 130, 256])
 def test_integer_probe_bit_exact(M, K):
     # power-of-two scales, X in {-1, 0, 1, 2}, codes over the whole int8 range: every partial sum is an exact integer
     N = 256
