@@ -176,7 +176,8 @@ int er_w4a16_gemm_static(const void* x_bf16, int64_t M, int64_t K, int64_t ldx_e
  *   weight.  er_unpack_codes(qweight, N, 2 K) returns the planes as (a - 8, b - 8).
  *   er_w8a16_gemm: Y = X . dequant^T with q * s never rounded: the W4 per-group kernel contracts both planes of a group
  *   against the same 128 columns of X with fp32 accumulation and applies the fp32 scales 16 s and s to the two partial
- *   sums; the offset of the stored nibbles (128 sum_k x) is removed on the fp32 sums or on the widened nibbles.  Every M >= 1.  Workspace: er_w8_gemm_workspace_bytes, counters zeroed once (er_gemm_workspace_init), shared with er_w4a16_gemm
+ *   sums; the offset of the stored nibbles (128 sum_k x) is removed on the fp32 sums or on the widened nibbles.  Every M >= 1.
+ *   Workspace: er_w8_gemm_workspace_bytes, counters zeroed once (er_gemm_workspace_init), shared with er_w4a16_gemm
  *   if large enough for both.  Arguments, alignment, errors, determinism as for er_quantize_pack / er_w4a16_gemm. */
 int er_quantize_pack8(const void* w_bf16, int64_t N, int64_t K, int64_t ldw_elems, int group, void* qweight_out,
                       void* scales_out, void* stream);
